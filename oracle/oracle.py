@@ -1,0 +1,161 @@
+"""ctypes front-end of the CPU oracle (oracle/z4c_oracle.cpp). TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this. It takes a parameter object with the attribute names of
+paper_2409_10383_b200.inputs.Z4cParams (duck-typed; nothing of the CUDA path is imported).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liboz4c.so")
+NF = 22
+
+
+class _OParams(C.Structure):
+    _fields_ = [("N", C.c_int32 * 3), ("bc", C.c_int32), ("dx", C.c_double), ("cfl", C.c_double),
+                ("kappa1", C.c_double), ("kappa2", C.c_double),
+                ("lapse_oplog", C.c_double), ("lapse_harmonic", C.c_double), ("lapse_advect", C.c_double),
+                ("shift_gamma", C.c_double), ("shift_eta", C.c_double), ("shift_advect", C.c_double),
+                ("ko_eps", C.c_double), ("chi_floor", C.c_double)]
+
+
+def build(force: bool = False) -> str:
+    """Compile liboz4c.so with the system g++ (-O2 -ffp-contract=off -fopenmp)."""
+    srcs = [os.path.join(_HERE, f) for f in ("z4c_oracle.cpp", "z4c_physics.hpp", "z4c_oracle.hpp")]
+    if (not force and os.path.exists(_LIB_PATH)
+            and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(s) for s in srcs)):
+        return _LIB_PATH
+    cxx = "/usr/bin/g++" if os.path.exists("/usr/bin/g++") else "g++"
+    cmd = [cxx, "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-fopenmp", "-shared",
+           "-o", _LIB_PATH, srcs[0]]
+    subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB_PATH
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB_PATH)
+        dp = C.POINTER(C.c_double)
+        pp = C.POINTER(_OParams)
+        L.oz4c_rhs.argtypes = [pp, dp, dp]
+        L.oz4c_enforce.argtypes = [pp, dp]
+        L.oz4c_enforce.restype = C.c_int
+        L.oz4c_step.argtypes = [pp, dp, C.c_int, C.c_int]
+        L.oz4c_step.restype = C.c_int
+        L.oz4c_step_textbook.argtypes = [pp, dp, C.c_int]
+        L.oz4c_inv_cbrt.argtypes = [C.c_double]
+        L.oz4c_inv_cbrt.restype = C.c_double
+        L.oz4c_constraints.argtypes = [pp, dp, dp, dp]
+        L.oz4c_stencil.argtypes = [pp, dp, C.c_int, C.c_int, C.c_int, dp]
+        L.oz4c_num_intermediates.restype = C.c_int
+        L.oz4c_intermediates.argtypes = [pp, dp, dp]
+        L.oz4c_count_flops.argtypes = [pp, dp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
+        L.oz4c_num_threads.restype = C.c_int
+        L.oz4c_set_num_threads.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def _op(p, N=None) -> _OParams:
+    o = _OParams()
+    NN = p.N if N is None else N
+    for a in range(3):
+        o.N[a] = int(NN[a])
+    o.bc = int(p.bc)
+    for name in ("dx", "cfl", "kappa1", "kappa2", "lapse_oplog", "lapse_harmonic", "lapse_advect",
+                 "shift_gamma", "shift_eta", "shift_advect", "ko_eps", "chi_floor"):
+        setattr(o, name, float(getattr(p, name)))
+    return o
+
+
+def _ptr(a: np.ndarray):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _N_of(u):
+    return (u.shape[-1], u.shape[-2], u.shape[-3])
+
+
+def num_threads() -> int:
+    return lib().oz4c_num_threads()
+
+
+def set_num_threads(n: int) -> None:
+    lib().oz4c_set_num_threads(int(n))
+
+
+def rhs(p, u: np.ndarray) -> np.ndarray:
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    out = np.empty_like(u)
+    lib().oz4c_rhs(C.byref(_op(p, _N_of(u))), _ptr(u), _ptr(out))
+    return out
+
+
+def enforce(p, u: np.ndarray):
+    u = np.array(u, dtype=np.float64, order="C", copy=True)
+    bad = lib().oz4c_enforce(C.byref(_op(p, _N_of(u))), _ptr(u))
+    return u, bad
+
+
+def step(p, u: np.ndarray, nsteps: int, do_enforce: bool = True):
+    u = np.array(u, dtype=np.float64, order="C", copy=True)
+    bad = lib().oz4c_step(C.byref(_op(p, _N_of(u))), _ptr(u), int(nsteps), int(do_enforce))
+    return u, bad
+
+
+def step_textbook(p, u: np.ndarray, nsteps: int) -> np.ndarray:
+    u = np.array(u, dtype=np.float64, order="C", copy=True)
+    lib().oz4c_step_textbook(C.byref(_op(p, _N_of(u))), _ptr(u), int(nsteps))
+    return u
+
+
+def inv_cbrt(x: float) -> float:
+    return lib().oz4c_inv_cbrt(float(x))
+
+
+def constraints(p, u: np.ndarray, percell: bool = False):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    out = np.zeros(8)
+    pc = np.empty((4,) + u.shape[1:]) if percell else None
+    lib().oz4c_constraints(C.byref(_op(p, _N_of(u))), _ptr(u), _ptr(out),
+                           _ptr(pc) if percell else None)
+    return (out, pc) if percell else out
+
+
+def stencil(p, f: np.ndarray, kind: int, a: int = 0, b: int = 0) -> np.ndarray:
+    f = np.ascontiguousarray(f, dtype=np.float64)
+    out = np.empty_like(f)
+    lib().oz4c_stencil(C.byref(_op(p, _N_of(f))), _ptr(f), kind, a, b, _ptr(out))
+    return out
+
+
+INTERMEDIATE = {"Rt": slice(0, 6), "Rchi": slice(6, 12), "DDalpha": slice(12, 18), "R": 18, "AA": 19,
+                "Gd": slice(20, 23), "ginv": slice(23, 29)}
+
+
+def intermediates(p, u: np.ndarray) -> np.ndarray:
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    nq = lib().oz4c_num_intermediates()
+    out = np.empty((nq,) + u.shape[1:])
+    lib().oz4c_intermediates(C.byref(_op(p, _N_of(u))), _ptr(u), _ptr(out))
+    return out
+
+
+def count_flops(p, u: np.ndarray, i: int, j: int, k: int):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    cnt = (C.c_longlong * 6)()
+    lib().oz4c_count_flops(C.byref(_op(p, _N_of(u))), _ptr(u), i, j, k, cnt)
+    return {"rhs": {"add": cnt[0], "mul": cnt[1], "div": cnt[2]},
+            "constraints": {"add": cnt[3], "mul": cnt[4], "div": cnt[5]}}

@@ -1,0 +1,414 @@
+"""Pins P1-P9 of SURVEY.md section 8(c): the CPU oracle against what the paper and the mathematics
+fix (closed forms, invariants, textbook definitions via sympy, convergence orders). CPU only."""
+from dataclasses import replace
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2409_10383_b200 import inputs as I
+from tests import analytic
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def box_params(N, lo, width, **kw):
+    """non-periodic box [lo, lo+width]^3 with N^3 cells (clamp BC; only cells >= 3 from the faces are checked)"""
+    return replace(I.Z4cParams(n=N, nb=(1, 1, 1), xmin=tuple(lo), dx=width / N, bc=1), **kw)
+
+
+def inner(a, m=3):
+    return a[..., m:-m, m:-m, m:-m]
+
+
+# ---------------------------------------------------------------- golden: the paper's printed parameters
+def test_paper_parameters_golden():
+    gold = json.load(open(os.path.join(GOLD, "paper_parameters.json")))
+    p = I.Z4cParams()
+    assert p.ko_eps == gold["ko_dissipation"]["value"]
+    assert p.kappa1 == gold["kappa1"]["value"] and p.kappa2 == gold["kappa2"]["value"]
+    assert p.cfl == gold["cfl"]["value"]
+    assert p.ng == gold["ghosts_4th_order"]["value"]
+    pw, uw, nsteps = I.config(1)
+    amp = np.abs(uw[I.GYY] - uw[I.CHI]).max()          # cell centres miss the crest by <= cos(pi/64)
+    assert 0.998 * gold["linear_wave_amplitude"]["value"] < amp <= gold["linear_wave_amplitude"]["value"]
+    # Eq. (6) of the paper: Q_n for factor-2 refinement and n = 4
+    assert gold["Q4_factor2"]["value"] == 2 ** 4
+
+
+# ---------------------------------------------------------------- P1 Minkowski
+def test_P1_minkowski_rhs_zero_and_state_fixed(oracle):
+    p = I.params_noise(8, (2, 1, 1))
+    u = I.minkowski(p)
+    assert np.all(oracle.rhs(p, u) == 0.0)
+    u2, bad = oracle.step(p, u, 3)
+    assert bad == 0 and np.array_equal(u2, u)
+    pw = replace(p, bc=1)
+    assert np.all(oracle.rhs(pw, u) == 0.0)
+
+
+# ---------------------------------------------------------------- P2 polynomial exactness
+def _poly_grid(N=12, h=0.37):
+    p = box_params(N, (-1.3, 0.4, 2.1), N * h, ko_eps=0.5)
+    z, y, x = I.cell_centres(p)
+    return p, x + 0 * y + 0 * z, y + 0 * x + 0 * z, z + 0 * x + 0 * y
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_P2_stencils_exact_on_degree4(oracle, axis):
+    p, xx, yy, zz = _poly_grid()
+    c = [xx, yy, zz][axis]
+    h = p.dx
+    for deg in range(0, 5):
+        f = c ** deg + 0.3 * c ** max(deg - 1, 0)
+        d1 = deg * c ** max(deg - 1, 0) + 0.3 * max(deg - 1, 0) * c ** max(deg - 2, 0)
+        d2 = deg * (deg - 1) * c ** max(deg - 2, 0) + 0.3 * max(deg - 1, 0) * max(deg - 2, 0) * c ** max(deg - 3, 0)
+        scale = np.abs(inner(f)).max() / h
+        for kind in (0, 3, 4):
+            err = np.abs(inner(oracle.stencil(p, f, kind, axis)) - inner(d1)).max()
+            assert err <= 2e-13 * scale, (kind, deg, err)
+        err = np.abs(inner(oracle.stencil(p, f, 1, axis)) - inner(d2)).max()
+        assert err <= 2e-13 * scale / h, (deg, err)
+    # KO annihilates degree <= 5
+    f = c ** 5 - 2 * c ** 3
+    assert np.abs(inner(oracle.stencil(p, f, 5))).max() <= 1e-11 * np.abs(f).max() / h
+
+
+def test_P2_leading_error_terms(oracle):
+    # centred-1st: -h^4 u^(5)/30 ; upwind: +h^4 u^(5)/20 on both sides ; KO = eps h^5 u^(6)/64
+    p, xx, yy, zz = _poly_grid()
+    h = p.dx
+    f5 = xx ** 5
+    exact = 5 * xx ** 4
+    e_c = inner(oracle.stencil(p, f5, 0, 0)) - inner(exact)
+    assert np.allclose(e_c, -h ** 4 * 120 / 30, rtol=1e-8, atol=0)
+    for kind in (3, 4):
+        e_u = inner(oracle.stencil(p, f5, kind, 0)) - inner(exact)
+        assert np.allclose(e_u, +h ** 4 * 120 / 20, rtol=1e-8, atol=0)
+    f6 = yy ** 6
+    ko = inner(oracle.stencil(p, f6, 5))
+    assert np.allclose(ko, p.ko_eps * h ** 5 * 720 / 64, rtol=1e-7, atol=0)
+
+
+def test_P2_mixed_derivative_exact_and_symmetric(oracle):
+    p, xx, yy, zz = _poly_grid()
+    c = [xx, yy, zz]
+    for a in range(3):
+        for b in range(a + 1, 3):
+            f = c[a] ** 4 * c[b] ** 3 + 2 * c[a] * c[b] ** 4 - c[a] ** 2 * c[b]
+            exact = 12 * c[a] ** 3 * c[b] ** 2 + 8 * c[b] ** 3 - 2 * c[a]
+            got = oracle.stencil(p, f, 2, a, b)
+            tol = 1e-12 * np.abs(f).max() / p.dx ** 2
+            assert np.abs(inner(got) - inner(exact)).max() <= tol
+            assert np.abs(inner(got) - inner(oracle.stencil(p, f, 2, b, a))).max() <= tol
+
+
+def test_P2_ko_sign_is_damping(oracle):
+    # highest-frequency mode (-1)^i: the KO term must oppose it (symbol -eps sin^6(kh/2)/h)
+    p = I.params_noise(8, (1, 1, 1), 0.1)
+    i = np.arange(8)
+    f = np.broadcast_to(((-1.0) ** i)[None, None, :], (8, 8, 8)).copy()
+    ko = oracle.stencil(p, f, 5)
+    assert np.allclose(ko, -p.ko_eps / p.dx * f, rtol=1e-13)
+
+
+# ---------------------------------------------------------------- P3 Ricci identity (sympy, textbook definition)
+def _ricci_error(oracle, N):
+    p = box_params(N, (0.1, -0.2, 0.3), 1.0, ko_eps=0.0)
+    z, y, x = I.cell_centres(p)
+    g, ric, gd = analytic.unimodular_metric()(x, y, z)
+    u = I.minkowski(p)
+    u[I.GXX:I.GZZ + 1] = g
+    u[I.GAMX:I.GAMZ + 1] = gd
+    q = oracle.intermediates(p, u)
+    m = 3 * N // 16                                   # same physical region at every resolution
+    assert np.abs(inner(q[oracle.INTERMEDIATE["Gd"]], m) - inner(gd, m)).max() < 5e-3 * (16 / N) ** 4
+    return np.abs(inner(q[oracle.INTERMEDIATE["Rt"]], m) - inner(ric, m)).max(axis=(1, 2, 3)), np.abs(ric).max()
+
+
+def test_P3_conformal_ricci_matches_textbook(oracle):
+    e16, scale = _ricci_error(oracle, 16)
+    e32, _ = _ricci_error(oracle, 32)
+    assert scale > 0.3                                # a non-trivial curvature
+    assert np.all(e32 < 2e-5 * scale)                 # converged to the textbook tensor ...
+    assert np.all(e16 / e32 > 11.0), e16 / e32        # ... at 4th order, every component
+
+
+# ---------------------------------------------------------------- P4 static isotropic Schwarzschild
+def _schw_iso(oracle, N):
+    p = box_params(N, (0.9, 0.6, -0.8), 1.6, ko_eps=0.0)
+    z, y, x = I.cell_centres(p)
+    r = np.sqrt(x * x + y * y + z * z)
+    psi = 1.0 + 0.5 / r
+    u = I.minkowski(p)
+    u[I.CHI] = psi ** -4
+    u[I.ALPHA] = (1.0 - 0.5 / r) / (1.0 + 0.5 / r)
+    rhs = oracle.rhs(p, u)
+    _, pc = oracle.constraints(p, u, percell=True)
+    m = 3 * N // 16                                   # same physical region at every resolution
+    return np.abs(inner(rhs, m)).max(axis=(1, 2, 3)), np.abs(inner(pc, m)).max(axis=(1, 2, 3))
+
+
+def test_P4_isotropic_schwarzschild_is_static(oracle):
+    r16, c16 = _schw_iso(oracle, 16)
+    r32, c32 = _schw_iso(oracle, 32)
+    assert np.all(r32 < 3e-6) and np.all(c32 < 3e-6)
+    big = r16 > 1e-12                                  # components that are not identically zero
+    assert big.sum() >= 7                              # Khat? no: A_ij (6) + Theta at least
+    assert np.all(r16[big] / r32[big] > 11.0), (r16, r32)
+    assert c16[0] / c32[0] > 11.0                      # Hamiltonian constraint -> 0 at 4th order
+
+
+def test_P4_brill_lindquist_hamiltonian_converges(oracle):
+    # configs 3-4 initial data are exact time-symmetric solutions: H -> 0 at 4th order
+    def hmax(N):
+        p = box_params(N, (0.55, 0.3, 0.2), 2.0)
+        u = I.puncture_data(p, (0.5, 0.5), ((3.0, 0.0, 0.0), (-3.0, 0.0, 0.0)))
+        _, pc = oracle.constraints(p, u, percell=True)
+        return np.abs(inner(pc[0], 3 * N // 16)).max()
+    h16, h32 = hmax(16), hmax(32)
+    assert h32 < 1e-5 and h16 / h32 > 11.0
+
+
+# ---------------------------------------------------------------- P5 Kerr-Schild Schwarzschild
+def _kerr_schild(oracle, N):
+    p = box_params(N, (0.9, -1.1, 1.6), 1.2, ko_eps=0.0, shift_eta=1.3)
+    z, y, x = I.cell_centres(p)
+    u, adv_alpha, adv_beta = analytic.kerr_schild()(x, y, z)
+    rhs = oracle.rhs(p, u)
+    _, pc = oracle.constraints(p, u, percell=True)
+    m = 3 * N // 16                                   # same physical region at every resolution
+
+    def inner(a):
+        return a[..., m:-m, m:-m, m:-m]
+    metric_sector = np.abs(inner(rhs[:18])).max(axis=(1, 2, 3))
+    # gauge sector by hand: d_t alpha = -2 alpha Khat + beta.d alpha ; d_t beta = Gam - eta beta + beta.d beta
+    ga = -2.0 * u[I.ALPHA] * u[I.KHAT] + adv_alpha
+    gb = u[I.GAMX:I.GAMZ + 1] - p.shift_eta * u[I.BETAX:] + adv_beta
+    gauge = np.array([np.abs(inner(rhs[I.ALPHA] - ga)).max()] +
+                     [np.abs(inner(rhs[I.BETAX + i] - gb[i])).max() for i in range(3)])
+    return metric_sector, np.abs(inner(pc)).max(axis=(1, 2, 3)), gauge, u
+
+
+def test_P5_kerr_schild_metric_sector_is_stationary(oracle):
+    m16, c16, g16, u = _kerr_schild(oracle, 16)
+    m32, c32, g32, _ = _kerr_schild(oracle, 32)
+    # the data are non-trivial in every sector
+    assert np.abs(u[I.KHAT]).max() > 0.1 and np.abs(u[I.AXX:I.AZZ + 1]).max() > 0.05
+    assert np.abs(u[I.BETAX:]).max() > 0.2 and np.abs(u[I.GAMX:I.GAMZ + 1]).max() > 0.05
+    assert np.all(m32 < 2e-6), m32
+    assert np.all(m16 / m32 > 10.0), m16 / m32
+    assert np.all(c32 < 2e-6) and np.all(c16 / c32 > 10.0), (c16, c32)
+    assert np.all(g32 < 2e-6) and np.all(g16 / g32 > 10.0), (g16, g32)
+
+
+# ---------------------------------------------------------------- P6 linear wave
+def _wave_run(oracle, N, ny=2):
+    p = I.params_linear_wave(N, N)
+    p = replace(p, nb=(1, 1, 1))
+    u0 = I.linear_wave_data(p)[:, :ny, :ny, :].copy()
+    nsteps = round(0.390625 / p.dt)                  # Q16: same physical time at every resolution
+    assert abs(nsteps * p.dt - 0.390625) < 1e-14
+    u1, bad = oracle.step(p, u0, nsteps)
+    assert bad == 0
+    exact = I.linear_wave_data(p, t=0.390625)[:, :ny, :ny, :]
+    return p, u1, exact
+
+
+def test_P6_pencil_equals_cube(oracle):
+    # data depending on x only: a periodic N x 2 x 2 pencil is the same problem as the N^3 cube
+    p = replace(I.params_linear_wave(16, 16), nb=(1, 1, 1))
+    u0 = I.linear_wave_data(p)
+    a, _ = oracle.step(p, u0, 2)
+    b, _ = oracle.step(p, u0[:, :2, :2, :].copy(), 2)
+    assert np.array_equal(a[:, :2, :2, :], b)
+
+
+def test_P6_linear_wave_converges_at_4th_order(oracle):
+    err = {}
+    for N in (32, 64, 128):
+        p, u1, exact = _wave_run(oracle, N)
+        err[N] = (np.abs(u1[I.GYY] - exact[I.GYY]).max(), np.abs(u1[I.GYY] - exact[I.GYY]).mean())
+        # the wave has actually moved: compare with t=0 data
+        assert np.abs(u1[I.GYY] - I.linear_wave_data(p)[I.GYY, :2, :2, :]).max() > 5e-9
+    assert 12.0 < err[32][0] / err[64][0] < 20.0, err
+    assert 12.0 < err[32][1] / err[64][1] < 20.0, err
+    # 64 -> 128 is "less clean": ~5e-15 approaches the 10 A^2 ~ 1e-15 plateau and round-off
+    assert err[128][0] < 0.5 * err[64][0] and err[128][0] < 1e-14 and err[64][1] / err[128][1] > 4.0, err
+    assert err[64][0] < 2e-5 * 1e-8                   # relative to the amplitude
+
+
+def test_P6_self_convergence_factor3(oracle):
+    # cell-centred grids share centres under refinement by 3: Q = 3^4 = 81 (Eq. 6)
+    sol = {}
+    for N in (16, 48, 144):
+        _, u1, _ = _wave_run(oracle, N)
+        sol[N] = u1[I.GYY, 0, 0, :] - u1[I.CHI, 0, 0, :]          # = chi*b: the wave itself
+    c = sol[16]
+    m = sol[48][1::3]
+    f = sol[144][4::9]
+    Q = np.abs(c - m).mean() / np.abs(m - f).mean()
+    assert 60.0 < Q < 100.0, Q
+
+
+# ---------------------------------------------------------------- P7 Theta / kappa couplings
+def test_P7_theta_kappa_terms(oracle):
+    p = replace(I.params_noise(8), kappa1=0.02, kappa2=0.3)
+    th = 1e-3
+    u = I.minkowski(p)
+    u[I.THETA] = th
+    r = oracle.rhs(p, u)
+    K = 2 * th
+    assert np.allclose(r[I.THETA], 0.5 * (2.0 / 3.0) * K * K - p.kappa1 * (2 + p.kappa2) * th, rtol=1e-13, atol=0)
+    assert np.allclose(r[I.KHAT], K * K / 3.0 + p.kappa1 * (1 - p.kappa2) * th, rtol=1e-13, atol=0)
+    assert np.allclose(r[I.CHI], (2.0 / 3.0) * K, rtol=1e-13, atol=0)
+    others = [f for f in range(I.NF) if f not in (I.THETA, I.KHAT, I.CHI)]
+    assert np.all(r[others] == 0.0)
+    # Gamma-tilde offset relaxes as -2 alpha kappa1 delta^i and drives the shift
+    u = I.minkowski(p)
+    d = np.array([1e-3, -2e-3, 3e-3])
+    for i in range(3):
+        u[I.GAMX + i] = d[i]
+    r = oracle.rhs(p, u)
+    for i in range(3):
+        assert np.allclose(r[I.GAMX + i], -2 * p.kappa1 * d[i], rtol=1e-13, atol=0)
+        assert np.allclose(r[I.BETAX + i], p.shift_gamma * d[i], rtol=1e-13, atol=0)
+
+
+def test_P7_lapse_conditions(oracle):
+    # uniform Khat on Minkowski: 1+log gives -2 alpha Khat, harmonic gives -alpha^2 Khat (Q7)
+    p = I.params_noise(8)
+    u = I.minkowski(p)
+    u[I.KHAT] = 1e-3
+    u[I.ALPHA] = 0.7
+    r = oracle.rhs(p, u)
+    assert np.allclose(r[I.ALPHA], -2 * 0.7 * 1e-3, rtol=1e-14)
+    ph = replace(p, lapse_oplog=0.0, lapse_harmonic=1.0)
+    assert np.allclose(oracle.rhs(ph, u)[I.ALPHA], -0.49 * 1e-3, rtol=1e-14)
+
+
+# ---------------------------------------------------------------- P8 robust stability (config 1)
+def test_P8_robust_stability(oracle):
+    p, u0, nsteps = I.config(0)
+    mink = I.minkowski(p)
+    d0 = np.abs(u0 - mink).max()
+    u, bad = oracle.step(p, u0, nsteps)
+    assert bad == 0 and np.all(np.isfinite(u))
+    # derivatives of grid-scale noise feed Gamt, At at the level d0/h = 10 d0 (h = 0.1): bounded by 50 d0 ...
+    d10 = np.abs(u - mink).max()
+    assert d10 < 50 * d0
+    u, bad = oracle.step(p, u, 240)
+    assert bad == 0 and np.all(np.isfinite(u))
+    # ... and decaying afterwards (KO dissipation + constraint damping): no growth over 250 steps
+    assert np.abs(u - mink).max() < d10
+
+
+# ---------------------------------------------------------------- P9 invariances
+def _permute_xy(u):
+    v = np.swapaxes(u, -1, -2).copy()
+    perm = list(range(I.NF))
+    sw = {I.GXX: I.GYY, I.GXZ: I.GYZ, I.AXX: I.AYY, I.AXZ: I.AYZ, I.GAMX: I.GAMY, I.BETAX: I.BETAY}
+    for a, b in sw.items():
+        perm[a], perm[b] = b, a
+    return v[perm]
+
+
+def _smooth_random_state(p, seed=7, amp=1e-2):
+    rng = np.random.default_rng(seed)
+    z, y, x = I.cell_centres(p)
+    L = p.N[0] * p.dx
+    u = I.minkowski(p)
+    for f in range(I.NF):
+        k = rng.integers(1, 3, size=3)
+        ph = rng.uniform(0, 2 * np.pi, size=3)
+        u[f] += amp * rng.uniform(0.5, 1.0) * (np.sin(2 * np.pi * k[0] * x / L + ph[0])
+                                               * np.cos(2 * np.pi * k[1] * y / L + ph[1])
+                                               + np.sin(2 * np.pi * k[2] * z / L + ph[2]))
+    return u
+
+
+def test_P9_axis_permutation(oracle):
+    p = I.params_noise(12, (1, 1, 1), 0.1)
+    u = _smooth_random_state(p)
+    r = oracle.rhs(p, u)
+    r2 = oracle.rhs(p, _permute_xy(u))
+    assert np.abs(_permute_xy(r2) - r).max() <= 1e-12 * np.abs(r).max()
+    assert np.abs(r).max() > 1e-3
+
+
+def test_P9_periodic_shift_is_bitwise(oracle):
+    p = I.params_noise(8, (2, 1, 1), 0.1)
+    u = _smooth_random_state(p, amp=1e-3)
+    a, _ = oracle.step(p, u, 1)
+    b, _ = oracle.step(p, np.roll(u, (1, 2, 3), axis=(1, 2, 3)), 1)
+    assert np.array_equal(np.roll(a, (1, 2, 3), axis=(1, 2, 3)), b)
+
+
+def test_P9_recurrence_equals_textbook_rk4(oracle):
+    p = I.params_noise(8, (1, 1, 1), 0.1)
+    u = _smooth_random_state(p, amp=1e-3)
+    a, _ = oracle.step(p, u, 3, do_enforce=False)
+    b = oracle.step_textbook(p, u, 3)
+    assert np.abs(a - b).max() < 2e-15 * 3 * 4
+    assert np.abs(a - u).max() > 1e-5
+
+
+# ---------------------------------------------------------------- O7 enforcement
+def test_O7_inv_cbrt_spec(oracle):
+    rng = np.random.default_rng(0)
+    xs = np.concatenate([np.exp(rng.uniform(np.log(1e-8), np.log(1e8), 2000)), 1 + rng.uniform(-1e-9, 1e-9, 2000),
+                         [1.0, 8.0, 0.125, 27.0]])
+    got = np.array([oracle.inv_cbrt(v) for v in xs])
+    ref = 1.0 / np.cbrt(xs.astype(np.longdouble))
+    assert np.abs(got / ref - 1).max() < 3e-16
+    assert oracle.inv_cbrt(1.0) == 1.0 and oracle.inv_cbrt(8.0) == 0.5
+
+
+def test_O7_enforcement(oracle):
+    p = I.params_noise(6, (1, 1, 1))
+    rng = np.random.default_rng(3)
+    u = I.minkowski(p) + 0.2 * rng.uniform(-1, 1, size=(I.NF, 6, 6, 6))
+    u[I.CHI, 0, 0, 0] = -0.5
+    A0 = u[I.AXX:I.AZZ + 1].copy()
+    g0 = u[I.GXX:I.GZZ + 1].copy()
+    v, bad = oracle.enforce(p, u)
+    assert bad == 0
+
+    def mat(s):
+        return np.array([[s[0], s[1], s[2]], [s[1], s[3], s[4]], [s[2], s[4], s[5]]]).transpose(2, 3, 4, 0, 1)
+    G, G0, A, A0m = mat(v[I.GXX:I.GZZ + 1]), mat(g0), mat(v[I.AXX:I.AZZ + 1]), mat(A0)
+    assert np.abs(np.linalg.det(G) - 1).max() < 1e-14
+    # metric only rescaled (conformal class preserved); A~ not rescaled, only its trace removed (Q5)
+    assert np.abs(G - G0 * (np.linalg.det(G0) ** (-1 / 3))[..., None, None]).max() < 1e-14
+    Gi = np.linalg.inv(G)
+    tr = np.einsum("...ij,...ij", Gi, A)
+    assert np.abs(tr).max() < 1e-14
+    tr0 = np.einsum("...ij,...ij", Gi, A0m)
+    assert np.abs(A - (A0m - G * tr0[..., None, None] / 3)).max() < 1e-14
+    assert v[I.CHI, 0, 0, 0] == p.chi_floor and np.array_equal(v[I.CHI].ravel()[1:], u[I.CHI].ravel()[1:])
+    untouched = [I.KHAT, I.GAMX, I.GAMY, I.GAMZ, I.THETA, I.ALPHA, I.BETAX, I.BETAY, I.BETAZ]
+    assert np.array_equal(v[untouched], u[untouched])
+    # bad metric is flagged
+    u[I.GXX, 1, 1, 1] = -5.0
+    assert oracle.enforce(p, u)[1] == 1
+
+
+def test_constraints_norm_definitions(oracle):
+    p = I.params_noise(8, (1, 1, 1))
+    u = _smooth_random_state(p, amp=1e-3)
+    out, pc = oracle.constraints(p, u, percell=True)
+    assert np.isclose(out[0], np.sqrt(np.mean(pc[0] ** 2)), rtol=1e-12)
+    assert np.isclose(out[1], np.abs(pc[0]).max(), rtol=1e-14)
+    assert np.isclose(out[4], np.sqrt(np.mean(u[I.THETA] ** 2)), rtol=1e-12)
+    assert np.isclose(out[5], np.abs(u[I.THETA]).max(), rtol=1e-14)
+    # |M| with a near-flat metric ~ euclidean norm of M_i
+    assert np.isclose(out[3], np.sqrt((pc[1:] ** 2).sum(0)).max(), rtol=5e-3)
+
+
+def test_flop_census(oracle):
+    p = I.params_noise(8, (1, 1, 1))
+    c = oracle.count_flops(p, _smooth_random_state(p), 3, 4, 5)
+    total = sum(c["rhs"].values())
+    assert 4000 < total < 9000, c
