@@ -1,0 +1,139 @@
+/* =====================================================================================
+ * z4c.h -- C ABI of the B200-native Z4c hot path (arXiv 2409.10383, "Performance-Portable
+ * Numerical Relativity with AthenaK").
+ *
+ * What the library computes: the fp64 Z4c right-hand side + classical RK4 step over ONE pack
+ * of same-level MeshBlocks on one GPU.  The paper describes the pieces at
+ *   PAPER.md:49-57  (section 2: Z4c formulation, Bona-Masso lapse, Gamma-driver shift; the
+ *                    equations themselves are deferred to Daszuta et al. 2021 -- the reading
+ *                    used here is written out in DESIGN.md / SURVEY.md section 8(c) O3-O7),
+ *   PAPER.md:63-65  (section 3: Mesh -> MeshBlock -> MeshBlockPack, ghost zones refilled at
+ *                    every Runge-Kutta stage),
+ *   PAPER.md:75-76, 84 (section 3.1: same-level ghost fill from the neighbour's active region),
+ *   PAPER.md:122-126 (section 3.2: cell-centred finite differences, order tied to ghost count),
+ *   PAPER.md:203    (section 4.3: RK4, CFL 0.25, KO dissipation 0.5, kappa1 = 0.02, kappa2 = 0).
+ *
+ * Conventions
+ *  - All functions return 0 (Z4C_OK) or a negative error code; they never throw or abort.
+ *    A message for the last failing call on a context is available from z4c_last_error().
+ *  - "device pointer" = CUDA device memory on the current device of the calling thread;
+ *    "host pointer" = ordinary host memory. Every pointer argument says which it is.
+ *  - Ownership: the CALLER owns the state buffer and the workspace buffer (e.g. torch tensors)
+ *    and must keep them alive and unaliased until z4c_destroy(). The library owns only the
+ *    host-side z4c_ctx and never allocates device memory.
+ *  - Stream semantics: every call enqueues its work on the CUDA stream given to z4c_create()
+ *    and returns without synchronising, except where stated ("synchronises").
+ *  - Determinism: results are bitwise reproducible run to run (no atomics on the state path).
+ *
+ * State layout (part of the contract so a caller may view the buffer as a tensor):
+ *    double y[22][N_b][m][m][m],  m = n + 2*ng,  x index fastest, block id
+ *    b = (bz*nb[1] + by)*nb[0] + bx;  local cell (i,j,k) of block b has global cell index
+ *    (bx*n + i - ng, ...).  Field order: 0 chi; 1-6 gt_xx,xy,xz,yy,yz,zz; 7 Khat;
+ *    8-13 At_xx,xy,xz,yy,yz,zz; 14-16 Gamt^x,y,z; 17 Theta; 18 alpha; 19-21 beta^x,y,z
+ *    (BASELINE.json north_star (a)).
+ * "Interior array" = double[22][Nz][Ny][Nx] in GLOBAL, block-free cell order (x fastest),
+ *    Nx = nb[0]*n etc.; cell centres x = xmin + (i + 1/2) dx.
+ * ===================================================================================== */
+#ifndef Z4C_H_
+#define Z4C_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define Z4C_NFIELDS 22
+
+enum {
+  Z4C_OK = 0,
+  Z4C_EINVAL = -1, /* bad argument / unsupported parameter */
+  Z4C_ECUDA = -2,  /* a CUDA runtime call or kernel launch failed */
+  Z4C_ESTATE = -3  /* device error flag set: non-finite value or det(gt) <= 0 seen by the stage update */
+};
+
+typedef struct z4c_ctx z4c_ctx; /* opaque, host memory, owned by the library */
+
+typedef struct {
+  int32_t n;      /* interior cells per MeshBlock edge (16, 32, 64 are the tuned sizes; any n >= 6 accepted) */
+  int32_t ng;     /* ghost zones per side; must be 3 (4th order by the rule at PAPER.md:124) */
+  int32_t nb[3];  /* block lattice (x,y,z); N_b = nb[0]*nb[1]*nb[2] */
+  int32_t bc;     /* 0 periodic; 1 outflow-copy: ghost = nearest interior cell, all six faces */
+  double xmin[3]; /* lower corner of the domain */
+  double dx;      /* cell size, same on all axes */
+  double cfl;     /* dt = cfl*dx */
+  double kappa1, kappa2;                             /* constraint damping */
+  double lapse_oplog, lapse_harmonic, lapse_advect;  /* d_t a = -(oplog*a + harmonic*a^2) Khat + advect*b^k d_k a */
+  double shift_gamma, shift_eta, shift_advect;       /* d_t b^i = gamma*Gamt^i - eta*b^i + advect*b^k d_k b^i */
+  double ko_eps;                                     /* Kreiss-Oliger strength (0.5) */
+  double chi_floor;                                  /* chi <- max(chi, chi_floor) in the stage update */
+} z4c_params;
+
+/* Bytes of the state buffer y: 22*N_b*m^3*8. Returns 0 if the parameters are invalid. */
+size_t z4c_state_bytes(const z4c_params* p);
+
+/* Bytes of the workspace (RK registers P and Q on interior cells, reduction scratch, error flag).
+ * Returns 0 if the parameters are invalid. */
+size_t z4c_workspace_bytes(const z4c_params* p);
+
+/* Create a context. p: host pointer (copied). d_state, d_work: device pointers of at least
+ * z4c_state_bytes / z4c_workspace_bytes bytes, 256-byte aligned. cuda_stream: a cudaStream_t
+ * passed as void* (NULL = legacy default stream). out: host pointer receiving the context.
+ * Zero-fills the workspace (asynchronously). Errors: Z4C_EINVAL, Z4C_ECUDA. */
+int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stream, z4c_ctx** out);
+
+/* Load initial data. interior: an interior array; host pointer (on_device = 0; pageable or
+ * pinned; the call synchronises) or device pointer (on_device = 1; async). The library never
+ * allocates device memory, so host input is staged through the RK register area of the
+ * workspace. The data are scattered into the pack, the algebraic constraints are enforced
+ * (det gt = 1, tr At = 0, chi floor), ghosts are filled, time is reset to 0
+ * and the RK registers are cleared. */
+int z4c_set_initial_data(z4c_ctx* ctx, const double* interior, int on_device);
+
+/* Advance nsteps classical RK4 steps: per stage  RHS -> stage update with
+ * enforcement -> ghost fill.  Asynchronous on the context's stream; no host synchronisation. */
+int z4c_step(z4c_ctx* ctx, int nsteps);
+
+/* Constraint diagnostics on the current state (ghosts must be valid, which every call above
+ * guarantees). out: host pointer to 8 doubles {H_rms, H_max, M_rms, M_max, Theta_rms,
+ * Theta_max, Z_rms, Z_max} over interior cells. d_percell: NULL or device pointer to
+ * double[4][Nz][Ny][Nx] receiving H, M_x, M_y, M_z. Synchronises the stream.
+ * Returns Z4C_ESTATE if the device error flag is set. */
+int z4c_constraints(z4c_ctx* ctx, double* out, double* d_percell);
+
+/* Inverse of z4c_set_initial_data: gather the interior cells of the pack into an interior
+ * array. host pointer (on_device = 0; synchronises; staged through the workspace, so the RK
+ * registers must not be live, i.e. not between stages -- always true between API calls) or
+ * device pointer (on_device = 1; async). */
+int z4c_get_interior(z4c_ctx* ctx, double* interior, int on_device);
+
+/* --- single stages of the hot path, exported for unit parity tests and profiling ------- */
+/* K1: refill every ghost cell of every block from the interior cell with the same global index
+ * after periodic wrap / outflow clamp. Async. */
+int z4c_fill_ghosts(z4c_ctx* ctx);
+/* K2 with c = 0, dt = 1: evaluate F(y) + Q_KO(y) on interior cells and write it as an interior
+ * array to d_out (device pointer). Overwrites RK register P. Async. */
+int z4c_eval_rhs(z4c_ctx* ctx, double* d_out);
+/* O7 enforcement alone on the interior cells of the pack, then ghost fill. Async. */
+int z4c_enforce(z4c_ctx* ctx);
+
+/* Block until the stream is idle and report the device error flag (Z4C_ESTATE if set). */
+int z4c_sync(z4c_ctx* ctx);
+
+/* Number of kernel launches the library has enqueued on this context so far. */
+int64_t z4c_launch_count(const z4c_ctx* ctx);
+/* Select the RHS kernel variant (0 = default tuned kernel, 1 = plain global-memory kernel).
+ * For A/B measurements; both variants compute the same values. */
+int z4c_set_variant(z4c_ctx* ctx, int variant);
+/* Enable (1) / disable (0) CUDA-graph replay of the RK4 step inside z4c_step. Default 0. */
+int z4c_use_graph(z4c_ctx* ctx, int enable);
+
+double z4c_time(const z4c_ctx* ctx);             /* simulation time = steps taken * dt */
+const char* z4c_last_error(const z4c_ctx* ctx);  /* host string owned by the context ("" if none) */
+void z4c_destroy(z4c_ctx* ctx);                  /* frees the host context only */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* Z4C_H_ */
