@@ -129,6 +129,11 @@ int z4c_set_variant(z4c_ctx* ctx, int variant);
 /* Enable (1) / disable (0) CUDA-graph replay of the RK4 step inside z4c_step. Default 0. */
 int z4c_use_graph(z4c_ctx* ctx, int enable);
 
+/* Fuse the ghost fill into the stage update ("ghost push": the thread that updates an interior cell also
+ * writes that cell's ghost images in the neighbouring blocks; same values as K1, one pass less over the
+ * state). 1 = fused (default), 0 = separate K3 and K1 launches. */
+int z4c_set_fused(z4c_ctx* ctx, int enable);
+
 double z4c_time(const z4c_ctx* ctx);             /* simulation time = steps taken * dt */
 const char* z4c_last_error(const z4c_ctx* ctx);  /* host string owned by the context ("" if none) */
 void z4c_destroy(z4c_ctx* ctx);                  /* frees the host context only */

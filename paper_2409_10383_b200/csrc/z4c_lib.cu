@@ -1,0 +1,386 @@
+// C ABI of the Z4c hot path (include/z4c.h): host-side context, launch sequencing of one RK4 step
+// (ghost zones are refilled at every Runge-Kutta stage), CUDA-graph replay, error reporting.
+// The library never allocates device memory and never touches the CPU oracle.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/z4c.h"
+#include "z4c_kernels.cuh"
+#include "z4c_rhs_tiled.cuh"
+
+using namespace z4c;
+
+struct z4c_ctx {
+  z4c_params prm;
+  Pack g;
+  FdConst fd;
+  SrcParams sp;
+  double dt;
+  double* y;        // device, caller-owned
+  double* P;        // device, workspace
+  double* Q;        // device, workspace
+  double* partial;  // device, workspace: K4 partials
+  double* result;   // device, workspace: 8 doubles
+  int* flag;        // device, workspace: error flag
+  cudaStream_t stream;
+  long long steps;
+  int64_t launches;
+  int variant;
+  int use_graph;
+  int fuse_ghosts;
+  cudaGraphExec_t graph_exec;
+  int graph_launches;
+  std::string err;
+};
+
+namespace {
+
+constexpr int K4_MAX_PARTS = 148 * 8;
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+bool valid_params(const z4c_params* p) {
+  if (!p) return false;
+  if (p->ng != NG || p->n < 2 * NG) return false;
+  if (p->nb[0] < 1 || p->nb[1] < 1 || p->nb[2] < 1) return false;
+  if (p->bc != 0 && p->bc != 1) return false;
+  if (!(p->dx > 0.0) || !std::isfinite(p->dx) || !(p->cfl > 0.0) || !std::isfinite(p->cfl)) return false;
+  const long long nblk = (long long)p->nb[0] * p->nb[1] * p->nb[2];
+  const long long m = p->n + 2 * NG;
+  if (nblk > (1LL << 24) || m > 1024) return false;
+  if (nblk * m * m * m > (1LL << 40)) return false;
+  return true;
+}
+
+Pack make_pack(const z4c_params& p) {
+  Pack g;
+  g.n = p.n;
+  g.m = p.n + 2 * NG;
+  g.nb[0] = p.nb[0]; g.nb[1] = p.nb[1]; g.nb[2] = p.nb[2];
+  g.nblk = p.nb[0] * p.nb[1] * p.nb[2];
+  g.bc = p.bc;
+  g.m2 = g.m * g.m;
+  g.n3 = g.n * g.n * g.n;
+  g.m3 = g.m * g.m * g.m;
+  g.fs = (long long)g.nblk * g.m3;
+  g.is = (long long)g.nblk * g.n3;
+  g.ncell = g.is;
+  return g;
+}
+
+int fail(z4c_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+int check_cuda(z4c_ctx* c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return Z4C_OK;
+  return fail(c, Z4C_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+int check_launch(z4c_ctx* c, const char* what) {
+  c->launches += 1;
+  return check_cuda(c, cudaGetLastError(), what);
+}
+
+int grid_for(long long total, int threads, long long cap = (1LL << 30)) {
+  long long b = (total + threads - 1) / threads;
+  if (b > cap) b = cap;
+  if (b < 1) b = 1;
+  return (int)b;
+}
+
+// ---- launch helpers (all asynchronous on c->stream) ---------------------------------------
+int launch_ghost_fill(z4c_ctx* c) {
+  const long long per_block = 6LL * c->g.m * c->g.m + 6LL * c->g.n * c->g.m + 6LL * c->g.n * c->g.n;
+  k_ghost_fill<<<grid_for(per_block * c->g.nblk, 256), 256, 0, c->stream>>>(c->g, c->y);
+  return check_launch(c, "k_ghost_fill");
+}
+
+int launch_rhs(z4c_ctx* c, double coef, double dt) {
+  const Pack& g = c->g;
+  if (c->variant == 0 && rhs_tiled_supported(g)) {
+    launch_rhs_tiled(g, c->y, c->P, c->fd, c->sp, coef, dt, c->stream);
+    return check_launch(c, "k_rhs_tiled");
+  }
+  const int tx = (g.n + K2_TX - 1) / K2_TX, ty = (g.n + K2_TY - 1) / K2_TY, tz = (g.n + K2_TZ - 1) / K2_TZ;
+  const long long nblocks = (long long)tx * ty * tz * g.nblk;
+  if (nblocks > 0x7fffffffLL) return fail(c, Z4C_EINVAL, "pack too large for one K2 launch");
+  k_rhs_global<<<(unsigned)nblocks, dim3(K2_TX, K2_TY, K2_TZ), 0, c->stream>>>(g, c->y, c->P, c->fd, c->sp, coef,
+                                                                                  dt, tx, ty, tz);
+  return check_launch(c, "k_rhs_global");
+}
+
+template <bool PUSH>
+void launch_stage_update_t(z4c_ctx* c, int stage, int grid) {
+  const Pack& g = c->g;
+  switch (stage) {
+    case 0: k_stage_update<0, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
+    case 1: k_stage_update<1, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
+    case 2: k_stage_update<2, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
+    case 3: k_stage_update<3, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
+    default: k_stage_update<4, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
+  }
+}
+
+// K3 (+ K1 when the ghost push is fused in)
+int launch_stage_update(z4c_ctx* c, int stage, bool push) {
+  const int grid = grid_for(c->g.ncell, 128);
+  if (push) launch_stage_update_t<true>(c, stage, grid);
+  else launch_stage_update_t<false>(c, stage, grid);
+  return check_launch(c, "k_stage_update");
+}
+
+// One classical RK4 step in the 3-register recurrence: per stage
+// K2 (P <- c_s P + dt L(y)) -> K3 (update + enforcement) -> K1 (ghost fill).
+int enqueue_step(z4c_ctx* c) {
+  static const double coef[4] = {0.0, 0.0, -0.5, 2.0};
+  for (int s = 1; s <= 4; ++s) {
+    int rc = launch_rhs(c, coef[s - 1], c->dt);
+    if (rc) return rc;
+    rc = launch_stage_update(c, s, c->fuse_ghosts != 0);
+    if (rc) return rc;
+    if (!c->fuse_ghosts) {
+      rc = launch_ghost_fill(c);
+      if (rc) return rc;
+    }
+  }
+  return Z4C_OK;
+}
+
+void drop_graph(z4c_ctx* c) {
+  if (c->graph_exec) {
+    cudaGraphExecDestroy(c->graph_exec);
+    c->graph_exec = nullptr;
+  }
+}
+
+int read_flag(z4c_ctx* c) {
+  int h = 0;
+  int rc = check_cuda(c, cudaMemcpyAsync(&h, c->flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream), "flag copy");
+  if (rc) return rc;
+  rc = check_cuda(c, cudaStreamSynchronize(c->stream), "stream sync");
+  if (rc) return rc;
+  if (h) return fail(c, Z4C_ESTATE, "device error flag set: non-finite value or det(gt) <= 0 in the stage update");
+  return Z4C_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t z4c_state_bytes(const z4c_params* p) {
+  if (!valid_params(p)) return 0;
+  const Pack g = make_pack(*p);
+  return (size_t)NF * (size_t)g.fs * sizeof(double);
+}
+
+size_t z4c_workspace_bytes(const z4c_params* p) {
+  if (!valid_params(p)) return 0;
+  const Pack g = make_pack(*p);
+  const size_t reg = align_up((size_t)NF * (size_t)g.is * sizeof(double));
+  return 2 * reg + align_up((size_t)K4_MAX_PARTS * 8 * sizeof(double)) + align_up(8 * sizeof(double)) + ALIGN;
+}
+
+int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stream, z4c_ctx** out) {
+  if (!out) return Z4C_EINVAL;
+  *out = nullptr;
+  if (!valid_params(p) || !d_state || !d_work) return Z4C_EINVAL;
+  if (((uintptr_t)d_state % ALIGN) || ((uintptr_t)d_work % ALIGN)) return Z4C_EINVAL;
+  z4c_ctx* c = new (std::nothrow) z4c_ctx();
+  if (!c) return Z4C_EINVAL;
+  c->prm = *p;
+  c->g = make_pack(*p);
+  const double h = p->dx;
+  c->fd.inv12h = 1.0 / (12.0 * h);
+  c->fd.inv12h2 = 1.0 / (12.0 * h * h);
+  c->fd.inv144h2 = 1.0 / (144.0 * h * h);
+  c->fd.ko = p->ko_eps / (64.0 * h);
+  c->sp.kappa1 = p->kappa1; c->sp.kappa2 = p->kappa2;
+  c->sp.lapse_oplog = p->lapse_oplog; c->sp.lapse_harmonic = p->lapse_harmonic; c->sp.lapse_advect = p->lapse_advect;
+  c->sp.shift_gamma = p->shift_gamma; c->sp.shift_eta = p->shift_eta; c->sp.shift_advect = p->shift_advect;
+  c->dt = p->cfl * p->dx;
+  c->y = (double*)d_state;
+  const size_t reg = align_up((size_t)NF * (size_t)c->g.is * sizeof(double));
+  char* w = (char*)d_work;
+  c->P = (double*)w;
+  c->Q = (double*)(w + reg);
+  c->partial = (double*)(w + 2 * reg);
+  c->result = (double*)(w + 2 * reg + align_up((size_t)K4_MAX_PARTS * 8 * sizeof(double)));
+  c->flag = (int*)((char*)c->result + align_up(8 * sizeof(double)));
+  c->stream = (cudaStream_t)cuda_stream;
+  c->steps = 0;
+  c->launches = 0;
+  c->variant = 0;
+  c->use_graph = 0;
+  c->fuse_ghosts = 1;
+  c->graph_exec = nullptr;
+  c->graph_launches = 0;
+  cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
+  if (e != cudaSuccess) {
+    delete c;
+    return Z4C_ECUDA;
+  }
+  *out = c;
+  return Z4C_OK;
+}
+
+int z4c_set_initial_data(z4c_ctx* c, const double* interior, int on_device) {
+  if (!c || !interior) return Z4C_EINVAL;
+  const size_t bytes = (size_t)NF * (size_t)c->g.ncell * sizeof(double);
+  const double* src = interior;
+  int rc;
+  if (!on_device) {
+    // stage through the RK register area (P and Q are contiguous and together hold 2x this size)
+    rc = check_cuda(c, cudaMemcpyAsync(c->P, interior, bytes, cudaMemcpyHostToDevice, c->stream), "H2D copy");
+    if (rc) return rc;
+    src = c->P;
+  }
+  // ghosts are overwritten below; clear the state first so no uninitialised value is ever read
+  rc = check_cuda(c, cudaMemsetAsync(c->y, 0, (size_t)NF * (size_t)c->g.fs * sizeof(double), c->stream), "memset");
+  if (rc) return rc;
+  k_layout<0><<<grid_for((long long)NF * c->g.ncell, 256, 148 * 32), 256, 0, c->stream>>>(c->g, c->y,
+                                                                                            (double*)src, NF);
+  rc = check_launch(c, "k_layout<0>");
+  if (rc) return rc;
+  rc = check_cuda(c, cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream), "memset flag");
+  if (rc) return rc;
+  rc = launch_stage_update(c, 0, false);
+  if (rc) return rc;
+  rc = launch_ghost_fill(c);
+  if (rc) return rc;
+  const size_t reg = align_up((size_t)NF * (size_t)c->g.is * sizeof(double));
+  rc = check_cuda(c, cudaMemsetAsync(c->P, 0, 2 * reg, c->stream), "memset registers");
+  if (rc) return rc;
+  c->steps = 0;
+  if (!on_device) return check_cuda(c, cudaStreamSynchronize(c->stream), "stream sync");
+  return Z4C_OK;
+}
+
+int z4c_step(z4c_ctx* c, int nsteps) {
+  if (!c || nsteps < 0) return Z4C_EINVAL;
+  if (c->use_graph) {
+    if (!c->graph_exec) {
+      cudaGraph_t graph = nullptr;
+      int rc = check_cuda(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal), "begin capture");
+      if (rc) return rc;
+      const int64_t before = c->launches;
+      rc = enqueue_step(c);
+      c->graph_launches = (int)(c->launches - before);
+      c->launches = before;
+      cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+      if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+      rc = check_cuda(c, e, "end capture");
+      if (rc) return rc;
+      e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+      cudaGraphDestroy(graph);
+      rc = check_cuda(c, e, "graph instantiate");
+      if (rc) { c->graph_exec = nullptr; return rc; }
+    }
+    for (int s = 0; s < nsteps; ++s) {
+      int rc = check_cuda(c, cudaGraphLaunch(c->graph_exec, c->stream), "graph launch");
+      if (rc) return rc;
+      c->launches += c->graph_launches;
+    }
+  } else {
+    for (int s = 0; s < nsteps; ++s) {
+      int rc = enqueue_step(c);
+      if (rc) return rc;
+    }
+  }
+  c->steps += nsteps;
+  return Z4C_OK;
+}
+
+int z4c_constraints(z4c_ctx* c, double* out, double* d_percell) {
+  if (!c || !out) return Z4C_EINVAL;
+  int nparts = grid_for(c->g.ncell, K4_THREADS, K4_MAX_PARTS);
+  k_constraints<<<nparts, K4_THREADS, 0, c->stream>>>(c->g, c->y, c->fd, c->sp, c->partial, d_percell);
+  int rc = check_launch(c, "k_constraints");
+  if (rc) return rc;
+  k_constraints_final<<<1, K4_THREADS, 0, c->stream>>>(c->partial, nparts, (double)c->g.ncell, c->result);
+  rc = check_launch(c, "k_constraints_final");
+  if (rc) return rc;
+  rc = check_cuda(c, cudaMemcpyAsync(out, c->result, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream),
+                  "D2H copy");
+  if (rc) return rc;
+  return read_flag(c);
+}
+
+int z4c_get_interior(z4c_ctx* c, double* interior, int on_device) {
+  if (!c || !interior) return Z4C_EINVAL;
+  const size_t bytes = (size_t)NF * (size_t)c->g.ncell * sizeof(double);
+  double* dst = on_device ? interior : c->P;
+  k_layout<1><<<grid_for((long long)NF * c->g.ncell, 256, 148 * 32), 256, 0, c->stream>>>(c->g, c->y, dst, NF);
+  int rc = check_launch(c, "k_layout<1>");
+  if (rc) return rc;
+  if (!on_device) {
+    rc = check_cuda(c, cudaMemcpyAsync(interior, c->P, bytes, cudaMemcpyDeviceToHost, c->stream), "D2H copy");
+    if (rc) return rc;
+    return check_cuda(c, cudaStreamSynchronize(c->stream), "stream sync");
+  }
+  return Z4C_OK;
+}
+
+int z4c_fill_ghosts(z4c_ctx* c) {
+  if (!c) return Z4C_EINVAL;
+  return launch_ghost_fill(c);
+}
+
+int z4c_eval_rhs(z4c_ctx* c, double* d_out) {
+  if (!c || !d_out) return Z4C_EINVAL;
+  int rc = launch_rhs(c, 0.0, 1.0);
+  if (rc) return rc;
+  k_layout<2><<<grid_for((long long)NF * c->g.ncell, 256, 148 * 32), 256, 0, c->stream>>>(c->g, c->P, d_out, NF);
+  return check_launch(c, "k_layout<2>");
+}
+
+int z4c_enforce(z4c_ctx* c) {
+  if (!c) return Z4C_EINVAL;
+  if (c->fuse_ghosts) return launch_stage_update(c, 0, true);
+  int rc = launch_stage_update(c, 0, false);
+  if (rc) return rc;
+  return launch_ghost_fill(c);
+}
+
+int z4c_sync(z4c_ctx* c) {
+  if (!c) return Z4C_EINVAL;
+  return read_flag(c);
+}
+
+int64_t z4c_launch_count(const z4c_ctx* c) { return c ? c->launches : 0; }
+
+int z4c_set_variant(z4c_ctx* c, int variant) {
+  if (!c || variant < 0 || variant > 1) return Z4C_EINVAL;
+  if (variant != c->variant) drop_graph(c);
+  c->variant = variant;
+  return Z4C_OK;
+}
+
+int z4c_use_graph(z4c_ctx* c, int enable) {
+  if (!c) return Z4C_EINVAL;
+  c->use_graph = enable ? 1 : 0;
+  if (!enable) drop_graph(c);
+  return Z4C_OK;
+}
+
+int z4c_set_fused(z4c_ctx* c, int enable) {
+  if (!c) return Z4C_EINVAL;
+  if ((enable ? 1 : 0) != c->fuse_ghosts) drop_graph(c);
+  c->fuse_ghosts = enable ? 1 : 0;
+  return Z4C_OK;
+}
+
+double z4c_time(const z4c_ctx* c) { return c ? (double)c->steps * c->dt : 0.0; }
+const char* z4c_last_error(const z4c_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+void z4c_destroy(z4c_ctx* c) {
+  if (!c) return;
+  drop_graph(c);
+  delete c;
+}
+
+}  // extern "C"

@@ -189,3 +189,25 @@ def config(idx: int):
         p = params_puncture(256, 32, 24.0, 1.0)
         return p, puncture_data(p, (0.5, 0.5), ((3.0, 0.0, 0.0), (-3.0, 0.0, 0.0))), 100
     raise ValueError("config 4 (load sweep) is parameterised: use params_noise + tiled_noise_data")
+
+
+# ---- generic strong-field test data (parity tests; not a BASELINE config) ------------------
+def smooth_random_data(p: Z4cParams, seed: int = 7, amplitude: float = 0.1, nmodes: int = 3) -> np.ndarray:
+    """Minkowski + a few random Fourier modes of the given amplitude on every field (periodic over the
+    domain, so usable with either boundary condition). All nonlinear terms, both upwind directions and all
+    tensor components are exercised; det(gt) stays > 0 for amplitude <~ 0.2."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    z, y, x = cell_centres(p)
+    N = p.N
+    L = [N[a] * p.dx for a in range(3)]
+    xs = [(x - p.xmin[0]) / L[0], (y - p.xmin[1]) / L[1], (z - p.xmin[2]) / L[2]]
+    u = minkowski(p)
+    for f in range(NF):
+        acc = np.zeros((N[2], N[1], N[0]))
+        for _ in range(nmodes):
+            k = rng.integers(-2, 3, size=3)
+            ph = rng.uniform(0.0, 2.0 * math.pi)
+            c = rng.uniform(-1.0, 1.0)
+            acc = acc + c * np.sin(2.0 * math.pi * (k[0] * xs[0] + k[1] * xs[1] + k[2] * xs[2]) + ph)
+        u[f] += (amplitude / nmodes) * acc
+    return u

@@ -1,0 +1,230 @@
+"""Thin Python binding of the C-ABI library (include/z4c.h): same names, argument marshalling only.
+
+PyTorch is used for device memory and streams and for nothing else: every step of the hot path runs in
+the CUDA kernels of `libz4c.so`. There is no CPU fallback: if the library is missing or no CUDA device is
+present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+NF = 22
+Z4C_OK, Z4C_EINVAL, Z4C_ECUDA, Z4C_ESTATE = 0, -1, -2, -3
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libz4c.so")
+
+# every symbol include/z4c.h declares
+SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_initial_data", "z4c_step",
+           "z4c_constraints", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
+           "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_time",
+           "z4c_last_error", "z4c_destroy"]
+
+
+class z4c_params(C.Structure):
+    """Mirror of `z4c_params` (include/z4c.h)."""
+    _fields_ = [("n", C.c_int32), ("ng", C.c_int32), ("nb", C.c_int32 * 3), ("bc", C.c_int32),
+                ("xmin", C.c_double * 3), ("dx", C.c_double), ("cfl", C.c_double),
+                ("kappa1", C.c_double), ("kappa2", C.c_double),
+                ("lapse_oplog", C.c_double), ("lapse_harmonic", C.c_double), ("lapse_advect", C.c_double),
+                ("shift_gamma", C.c_double), ("shift_eta", C.c_double), ("shift_advect", C.c_double),
+                ("ko_eps", C.c_double), ("chi_floor", C.c_double)]
+
+
+def make_params(p) -> z4c_params:
+    """From any object with the attribute names of `inputs.Z4cParams`."""
+    o = z4c_params()
+    o.n, o.ng, o.bc = int(p.n), int(p.ng), int(p.bc)
+    for a in range(3):
+        o.nb[a] = int(p.nb[a])
+        o.xmin[a] = float(p.xmin[a])
+    for name in ("dx", "cfl", "kappa1", "kappa2", "lapse_oplog", "lapse_harmonic", "lapse_advect",
+                 "shift_gamma", "shift_eta", "shift_advect", "ko_eps", "chi_floor"):
+        setattr(o, name, float(getattr(p, name)))
+    return o
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libz4c.so and declare the prototypes. Raises if the library is not built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it with `python -m paper_2409_10383_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    pp, vp, dp = C.POINTER(z4c_params), C.c_void_p, C.c_void_p
+    L.z4c_state_bytes.argtypes = [pp]
+    L.z4c_state_bytes.restype = C.c_size_t
+    L.z4c_workspace_bytes.argtypes = [pp]
+    L.z4c_workspace_bytes.restype = C.c_size_t
+    L.z4c_create.argtypes = [pp, vp, vp, vp, C.POINTER(vp)]
+    L.z4c_set_initial_data.argtypes = [vp, dp, C.c_int]
+    L.z4c_step.argtypes = [vp, C.c_int]
+    L.z4c_constraints.argtypes = [vp, C.POINTER(C.c_double), dp]
+    L.z4c_get_interior.argtypes = [vp, dp, C.c_int]
+    L.z4c_fill_ghosts.argtypes = [vp]
+    L.z4c_eval_rhs.argtypes = [vp, dp]
+    L.z4c_enforce.argtypes = [vp]
+    L.z4c_sync.argtypes = [vp]
+    L.z4c_launch_count.argtypes = [vp]
+    L.z4c_launch_count.restype = C.c_int64
+    L.z4c_set_variant.argtypes = [vp, C.c_int]
+    L.z4c_use_graph.argtypes = [vp, C.c_int]
+    L.z4c_set_fused.argtypes = [vp, C.c_int]
+    L.z4c_time.argtypes = [vp]
+    L.z4c_time.restype = C.c_double
+    L.z4c_last_error.argtypes = [vp]
+    L.z4c_last_error.restype = C.c_char_p
+    L.z4c_destroy.argtypes = [vp]
+    L.z4c_destroy.restype = None
+    for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_get_interior",
+               "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
+               "z4c_set_fused"):
+        getattr(L, fn).restype = C.c_int
+    if path == LIB_PATH:
+        _lib = L
+    return L
+
+
+class Z4cError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"z4c error {code}: {msg}")
+        self.code = code
+
+
+class Z4c:
+    """Owns the device buffers (torch tensors) and a library context; methods are 1:1 with the C ABI."""
+
+    def __init__(self, p, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the Z4c path has no CPU fallback")
+        self.torch = torch
+        self.lib = load_library()
+        self.p = p
+        self.cp = make_params(p)
+        self.device = torch.device(device)
+        sb = self.lib.z4c_state_bytes(C.byref(self.cp))
+        wb = self.lib.z4c_workspace_bytes(C.byref(self.cp))
+        if sb == 0 or wb == 0:
+            raise Z4cError(Z4C_EINVAL, "invalid parameters")
+        m = p.n + 2 * p.ng
+        nblk = p.nb[0] * p.nb[1] * p.nb[2]
+        with torch.cuda.device(self.device):
+            self.state = torch.empty((NF, nblk, m, m, m), dtype=torch.float64, device=self.device)
+            self.work = torch.empty(wb // 8, dtype=torch.float64, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            assert self.state.numel() * 8 == sb
+            h = C.c_void_p()
+            rc = self.lib.z4c_create(C.byref(self.cp), self.state.data_ptr(), self.work.data_ptr(),
+                                     self.stream.cuda_stream, C.byref(h))
+        if rc != 0:
+            raise Z4cError(rc, "z4c_create failed")
+        self.h = h
+
+    # -- helpers ----------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise Z4cError(rc, self.lib.z4c_last_error(self.h).decode())
+
+    @property
+    def interior_shape(self):
+        N = self.p.N
+        return (NF, N[2], N[1], N[0])
+
+    # -- the ABI ----------------------------------------------------------------------------
+    def set_initial_data(self, interior):
+        """interior: numpy float64 [22][Nz][Ny][Nx] (host) or a CUDA float64 torch tensor of that shape."""
+        torch = self.torch
+        with torch.cuda.device(self.device):
+            if isinstance(interior, np.ndarray):
+                a = np.ascontiguousarray(interior, dtype=np.float64)
+                assert a.shape == self.interior_shape
+                self._check(self.lib.z4c_set_initial_data(self.h, a.ctypes.data, 0))
+            else:
+                t = interior
+                assert t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == self.interior_shape
+                if t.is_cuda:
+                    self._check(self.lib.z4c_set_initial_data(self.h, t.data_ptr(), 1))
+                else:
+                    self._check(self.lib.z4c_set_initial_data(self.h, t.data_ptr(), 0))
+
+    def step(self, nsteps: int = 1):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_step(self.h, int(nsteps)))
+
+    def constraints(self, percell: bool = False):
+        out = (C.c_double * 8)()
+        pc = None
+        with self.torch.cuda.device(self.device):
+            if percell:
+                pc = self.torch.empty((4,) + self.interior_shape[1:], dtype=self.torch.float64, device=self.device)
+            self._check(self.lib.z4c_constraints(self.h, out, pc.data_ptr() if percell else None))
+        res = np.array(list(out))
+        return (res, pc.cpu().numpy()) if percell else res
+
+    def get_interior(self, out=None) -> np.ndarray:
+        """Host copy of the interior cells (numpy). If `out` is a CUDA tensor, fills it on the device instead."""
+        with self.torch.cuda.device(self.device):
+            if out is not None and not isinstance(out, np.ndarray):
+                assert out.is_cuda and out.dtype == self.torch.float64 and out.is_contiguous()
+                self._check(self.lib.z4c_get_interior(self.h, out.data_ptr(), 1))
+                return out
+            a = out if out is not None else np.empty(self.interior_shape, dtype=np.float64)
+            assert a.flags["C_CONTIGUOUS"] and a.dtype == np.float64 and a.shape == self.interior_shape
+            self._check(self.lib.z4c_get_interior(self.h, a.ctypes.data, 0))
+            return a
+
+    def fill_ghosts(self):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_fill_ghosts(self.h))
+
+    def eval_rhs(self) -> np.ndarray:
+        with self.torch.cuda.device(self.device):
+            out = self.torch.empty(self.interior_shape, dtype=self.torch.float64, device=self.device)
+            self._check(self.lib.z4c_eval_rhs(self.h, out.data_ptr()))
+            self._check(self.lib.z4c_sync(self.h))
+        return out.cpu().numpy()
+
+    def enforce(self):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_enforce(self.h))
+
+    def sync(self):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_sync(self.h))
+
+    def launch_count(self) -> int:
+        return int(self.lib.z4c_launch_count(self.h))
+
+    def set_variant(self, v: int):
+        self._check(self.lib.z4c_set_variant(self.h, int(v)))
+
+    def use_graph(self, enable: bool):
+        self._check(self.lib.z4c_use_graph(self.h, int(bool(enable))))
+
+    def set_fused(self, enable: bool):
+        self._check(self.lib.z4c_set_fused(self.h, int(bool(enable))))
+
+    def time(self) -> float:
+        return float(self.lib.z4c_time(self.h))
+
+    def close(self):
+        if getattr(self, "h", None) is not None and self.h:
+            self.torch.cuda.synchronize(self.device)
+            self.lib.z4c_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

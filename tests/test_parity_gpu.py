@@ -1,0 +1,239 @@
+"""GPU parity tests: every call goes through the C ABI (paper_2409_10383_b200.z4c) and is compared with the
+CPU oracle element by element on the same seeded inputs. Tolerances:
+integer/index work (ghost fill, layout) bit-exact; floating point <= 1e-12 of max(|field|_max, S) after one
+step and <= 1e-10 after 100 steps (BASELINE.json north_star), S = perturbation scale (reading Q13)."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from paper_2409_10383_b200 import inputs as I
+from tests.parity import padded_reference, perturbation_scale, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_1STEP = 1e-12
+TOL_100STEP = 1e-10
+
+
+@pytest.fixture(scope="module")
+def Z():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2409_10383_b200 import build, z4c
+    build.build()
+    return z4c
+
+
+def make(Z, p, u, **kw):
+    sim = Z.Z4c(p)
+    if "variant" in kw:
+        sim.set_variant(kw["variant"])
+    if "fused" in kw:
+        sim.set_fused(kw["fused"])
+    if "graph" in kw:
+        sim.use_graph(kw["graph"])
+    sim.set_initial_data(u)
+    return sim
+
+
+CASES = {
+    "noise_1blk": lambda: (I.params_noise(16, (1, 1, 1)), "noise"),
+    "noise_ragged": lambda: (I.params_noise(10, (2, 3, 1)), "noise"),
+    "smooth_periodic": lambda: (I.params_noise(12, (2, 1, 2), dx=0.05), "smooth"),
+    "smooth_outflow": lambda: (replace(I.params_noise(16, (1, 2, 2), dx=0.05), bc=1, shift_eta=1.0), "smooth"),
+    "smooth_n32": lambda: (I.params_noise(32, (1, 1, 1), dx=0.03), "smooth"),
+}
+
+
+def case_data(name):
+    p, kind = CASES[name]()
+    u = I.noise_data(p, 1234) if kind == "noise" else I.smooth_random_data(p, 11, 0.1)
+    return p, u
+
+
+# ------------------------------------------------------------------------------ S1 + layout + E
+@pytest.mark.parametrize("name", list(CASES))
+def test_ghost_fill_and_enforcement_bitwise(Z, oracle, name):
+    p, u = case_data(name)
+    sim = make(Z, p, u)
+    ue, bad = oracle.enforce(p, u)
+    assert bad == 0
+    got = sim.state.cpu().numpy()
+    ref = padded_reference(ue, p)
+    # conformal metric: bit-exact (fixed IEEE sequence, reading R-E1); everything untouched by E: bit-exact
+    exact = [f for f in range(I.NF) if not (I.AXX <= f <= I.AZZ)]
+    assert np.array_equal(got[exact], ref[exact])
+    assert np.abs(got[I.AXX:I.AZZ + 1] - ref[I.AXX:I.AZZ + 1]).max() <= 4e-16 * max(1e-300, np.abs(ref[I.AXX:I.AZZ + 1]).max())
+    # the get_interior round trip is the inverse layout map
+    assert np.array_equal(sim.get_interior()[exact], ue[exact])
+    # standalone K1 after scrambling the ghosts
+    import torch
+    interior = sim.get_interior()
+    sim.state.fill_(float("nan"))
+    sim.set_fused(False)
+    sim.set_initial_data(interior)
+    assert np.array_equal(sim.state.cpu().numpy()[exact], ref[exact])
+    sim.close()
+
+
+def test_chi_floor_and_error_flag(Z, oracle):
+    p = replace(I.params_noise(8, (1, 1, 1)), chi_floor=1e-3)
+    u = I.smooth_random_data(p, 3, 0.05)
+    u[I.CHI, 2, 3, 4] = 1e-9
+    u[I.CHI, 5, 5, 5] = -0.5
+    sim = make(Z, p, u)
+    ue, bad = oracle.enforce(p, u)
+    got = sim.get_interior()
+    assert got[I.CHI, 2, 3, 4] == 1e-3 and got[I.CHI, 5, 5, 5] == 1e-3
+    assert np.array_equal(got[I.CHI], ue[I.CHI])
+    sim.sync()
+    u[I.GXX, 1, 1, 1] = -1.0      # det <= 0 -> error flag, reported as Z4C_ESTATE
+    sim.set_initial_data(u)
+    with pytest.raises(Z.Z4cError) as e:
+        sim.sync()
+    assert e.value.code == Z.Z4C_ESTATE
+    assert oracle.enforce(p, u)[1] == 1
+    sim.close()
+
+
+# ------------------------------------------------------------------------------ S2 + S3
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("name", list(CASES))
+def test_rhs_parity(Z, oracle, name, variant):
+    p, u = case_data(name)
+    sim = make(Z, p, u, variant=variant)
+    ue, _ = oracle.enforce(p, u)
+    ref = oracle.rhs(p, ue)
+    got = sim.eval_rhs()
+    err = rel_err(got, ref, float(np.abs(ref).max()) * 1e-3)
+    assert err.max() <= TOL_1STEP, dict(zip(I.FIELD_NAMES, err))
+    sim.close()
+
+
+def test_rhs_minkowski_exact_zero(Z):
+    p = I.params_noise(16, (2, 1, 1))
+    for variant in (0, 1):
+        sim = make(Z, p, I.minkowski(p), variant=variant)
+        assert np.all(sim.eval_rhs() == 0.0)
+        sim.step(3)
+        assert np.array_equal(sim.get_interior(), I.minkowski(p))
+        sim.close()
+
+
+# ------------------------------------------------------------------------------ whole step
+@pytest.mark.parametrize("name", list(CASES))
+def test_one_step_parity(Z, oracle, name):
+    p, u = case_data(name)
+    ref, bad = oracle.step(p, u, 1)
+    assert bad == 0
+    S = perturbation_scale(ref, p)
+    results = []
+    for kw in ({"variant": 0, "fused": True}, {"variant": 1, "fused": False}, {"variant": 0, "fused": True, "graph": True}):
+        sim = make(Z, p, u, **kw)
+        sim.step(1)
+        sim.sync()
+        got = sim.get_interior()
+        err = rel_err(got, ref, S)
+        assert err.max() <= TOL_1STEP, (kw, dict(zip(I.FIELD_NAMES, err)))
+        assert abs(sim.time() - p.dt) < 1e-15
+        results.append((got, sim.state.cpu().numpy()))
+        sim.close()
+    # CUDA-graph replay is the same launches: bitwise equal, ghosts included
+    assert np.array_equal(results[0][1], results[2][1])
+    # ghosts are consistent with the interior after the step (fused push == definition O2)
+    assert np.array_equal(results[0][1], padded_reference(results[0][0], p))
+    assert np.array_equal(results[1][1], padded_reference(results[1][0], p))
+
+
+def test_fused_push_equals_separate_ghost_fill_bitwise(Z):
+    for name in ("noise_ragged", "smooth_outflow"):
+        p, u = case_data(name)
+        a = make(Z, p, u, fused=True)
+        b = make(Z, p, u, fused=False)
+        a.step(3)
+        b.step(3)
+        assert np.array_equal(a.state.cpu().numpy(), b.state.cpu().numpy())
+        a.close()
+        b.close()
+
+
+def test_config1_robust_stability_10_steps(Z, oracle):
+    """BASELINE.json configs[0] in full."""
+    p, u, nsteps = I.config(0)
+    ref, bad = oracle.step(p, u, nsteps)
+    assert bad == 0
+    sim = make(Z, p, u, graph=True)
+    sim.step(nsteps)
+    sim.sync()
+    got = sim.get_interior()
+    S = perturbation_scale(ref, p)
+    err = rel_err(got, ref, S)
+    assert err.max() <= TOL_100STEP, dict(zip(I.FIELD_NAMES, err))
+    # P8: stays bounded
+    assert perturbation_scale(got, p) <= 10 * max(perturbation_scale(u, p), 1e-9)
+    sim.close()
+
+
+def test_linear_wave_100_steps_small(Z, oracle):
+    """BASELINE.json configs[1] at 32^3 (8 blocks of 16^3), 50 steps to the common time, then to 100 steps."""
+    p = I.params_linear_wave(32, 16)
+    u = I.linear_wave_data(p)
+    sim = make(Z, p, u)
+    ref = u
+    for target in (1, 50, 100):
+        done = int(round(sim.time() / p.dt))
+        ref, bad = oracle.step(p, ref, target - done)
+        sim.step(target - done)
+        sim.sync()
+        got = sim.get_interior()
+        S = perturbation_scale(ref, p)
+        err = rel_err(got, ref, S)
+        tol = TOL_1STEP if target == 1 else TOL_100STEP
+        assert err.max() <= tol, (target, dict(zip(I.FIELD_NAMES, err)))
+    sim.close()
+
+
+def test_puncture_small_20_steps(Z, oracle):
+    """BASELINE.json configs[2] shrunk to 32^3 cells (8 blocks of 16^3), outflow-copy boundary."""
+    p = I.params_puncture(32, 16, 8.0, 2.0)
+    u = I.puncture_data(p)
+    sim = make(Z, p, u)
+    ref = u
+    for target in (1, 20):
+        done = int(round(sim.time() / p.dt))
+        ref, bad = oracle.step(p, ref, target - done)
+        assert bad == 0
+        sim.step(target - done)
+        sim.sync()
+        got = sim.get_interior()
+        err = rel_err(got, ref, perturbation_scale(ref, p))
+        assert err.max() <= (TOL_1STEP if target == 1 else TOL_100STEP), (target, dict(zip(I.FIELD_NAMES, err)))
+    sim.close()
+
+
+# ------------------------------------------------------------------------------ S5
+@pytest.mark.parametrize("name", ["smooth_periodic", "smooth_outflow", "noise_ragged"])
+def test_constraints_parity(Z, oracle, name):
+    p, u = case_data(name)
+    sim = make(Z, p, u)
+    ue, _ = oracle.enforce(p, u)
+    ref, ref_pc = oracle.constraints(p, ue, percell=True)
+    got, got_pc = sim.constraints(percell=True)
+    scale = np.abs(ref_pc).max()
+    assert np.abs(got_pc - ref_pc).max() <= 1e-12 * scale
+    assert np.all(np.abs(got - ref) <= 1e-12 * np.maximum(np.abs(ref), scale * 1e-3))
+    again = sim.constraints()
+    assert np.array_equal(again, got)        # fixed-order reductions: bitwise reproducible
+    sim.close()
+
+
+def test_run_to_run_determinism(Z):
+    p, u = case_data("smooth_outflow")
+    outs = []
+    for _ in range(2):
+        sim = make(Z, p, u)
+        sim.step(5)
+        outs.append(sim.state.cpu().numpy())
+        sim.close()
+    assert np.array_equal(outs[0], outs[1])
