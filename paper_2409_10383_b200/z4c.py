@@ -121,7 +121,9 @@ class Z4c:
         with torch.cuda.device(self.device):
             self.state = torch.empty((NF, nblk, m, m, m), dtype=torch.float64, device=self.device)
             self.work = torch.empty(wb // 8, dtype=torch.float64, device=self.device)
-            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            # a dedicated non-default stream: CUDA-graph capture is not allowed on the legacy default stream
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+            torch.cuda.synchronize(self.device)
             assert self.state.numel() * 8 == sb
             h = C.c_void_p()
             rc = self.lib.z4c_create(C.byref(self.cp), self.state.data_ptr(), self.work.data_ptr(),
