@@ -118,6 +118,17 @@ int z4c_eval_rhs(z4c_ctx* ctx, double* d_out);
 /* O7 enforcement alone on the interior cells of the pack, then ghost fill. Async. */
 int z4c_enforce(z4c_ctx* ctx);
 
+/* --- measurement aids (bench.py) -------------------------------------------------------- */
+/* z4c_step with a CUDA event recorded on the context's stream between every pair of kernels.
+ * ms_out: host pointer to 3 doubles receiving the summed device time in milliseconds of
+ * {K2 RHS, K3 stage update (+ghost push), K1 ghost fill}. Synchronises. Never uses graph replay. */
+int z4c_step_timed(z4c_ctx* ctx, int nsteps, double* ms_out);
+/* FP64 pipe probe: runs a dependency-free DFMA loop on every SM of the current device (8 CTAs of 256
+ * threads per SM, 8 chains per thread, `iters` iterations) and returns the achieved TFLOP/s (2 flop per
+ * DFMA) in *tflops_out (host pointer). d_scratch: device pointer to >= 8 bytes. Synchronises. This is the
+ * measured denominator of the "alu" roofline (MEASURED_PEAKS.json has no FP64 figure). */
+int z4c_probe_fp64(void* cuda_stream, void* d_scratch, int iters, double* tflops_out);
+
 /* Block until the stream is idle and report the device error flag (Z4C_ESTATE if set). */
 int z4c_sync(z4c_ctx* ctx);
 

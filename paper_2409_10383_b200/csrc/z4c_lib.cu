@@ -151,6 +151,54 @@ int enqueue_step(z4c_ctx* c) {
   return Z4C_OK;
 }
 
+// The same launches as enqueue_step with a CUDA event between every pair of kernels, for per-kernel
+// durations measured on the launching stream. ms[0..2] += time in K2, K3, K1.
+int enqueue_step_timed(z4c_ctx* c, cudaEvent_t* ev, double* ms) {
+  static const double coef[4] = {0.0, 0.0, -0.5, 2.0};
+  int ne = 0;
+  int kind[16];
+  int rc = check_cuda(c, cudaEventRecord(ev[ne++], c->stream), "event record");
+  if (rc) return rc;
+  for (int s = 1; s <= 4; ++s) {
+    rc = launch_rhs(c, coef[s - 1], c->dt);
+    if (rc) return rc;
+    kind[ne] = 0;
+    cudaEventRecord(ev[ne++], c->stream);
+    rc = launch_stage_update(c, s, c->fuse_ghosts != 0);
+    if (rc) return rc;
+    kind[ne] = 1;
+    cudaEventRecord(ev[ne++], c->stream);
+    if (!c->fuse_ghosts) {
+      rc = launch_ghost_fill(c);
+      if (rc) return rc;
+      kind[ne] = 2;
+      cudaEventRecord(ev[ne++], c->stream);
+    }
+  }
+  rc = check_cuda(c, cudaEventSynchronize(ev[ne - 1]), "event sync");
+  if (rc) return rc;
+  for (int e = 1; e < ne; ++e) {
+    float t = 0.f;
+    rc = check_cuda(c, cudaEventElapsedTime(&t, ev[e - 1], ev[e]), "event elapsed");
+    if (rc) return rc;
+    ms[kind[e]] += (double)t;
+  }
+  return Z4C_OK;
+}
+
+__global__ void __launch_bounds__(256) k_probe_dfma(double* out, int iters) {
+  // 8 independent dependency chains of DFMA per thread: measures the FP64 pipe's issue rate
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0,
+         a6 = a0 + 6.0, a7 = a0 + 7.0;
+  const double m = 1.0000001, b = 1e-9;
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+    a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+  }
+  const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (r == 123.456) out[0] = r;   // never true: keeps the loop alive
+}
+
 void drop_graph(z4c_ctx* c) {
   if (c->graph_exec) {
     cudaGraphExecDestroy(c->graph_exec);
@@ -344,6 +392,42 @@ int z4c_enforce(z4c_ctx* c) {
   int rc = launch_stage_update(c, 0, false);
   if (rc) return rc;
   return launch_ghost_fill(c);
+}
+
+int z4c_step_timed(z4c_ctx* c, int nsteps, double* ms_out) {
+  if (!c || nsteps < 0 || !ms_out) return Z4C_EINVAL;
+  cudaEvent_t ev[16];
+  for (int e = 0; e < 16; ++e)
+    if (cudaEventCreate(&ev[e]) != cudaSuccess) return fail(c, Z4C_ECUDA, "event create");
+  ms_out[0] = ms_out[1] = ms_out[2] = 0.0;
+  int rc = Z4C_OK;
+  for (int s = 0; s < nsteps && rc == Z4C_OK; ++s) rc = enqueue_step_timed(c, ev, ms_out);
+  for (int e = 0; e < 16; ++e) cudaEventDestroy(ev[e]);
+  if (rc == Z4C_OK) c->steps += nsteps;
+  return rc;
+}
+
+int z4c_probe_fp64(void* cuda_stream, void* d_scratch, int iters, double* tflops_out) {
+  if (!d_scratch || !tflops_out || iters < 1) return Z4C_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return Z4C_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return Z4C_ECUDA;
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return Z4C_ECUDA;
+  const int grid = sms * 8, threads = 256;
+  k_probe_dfma<<<grid, threads, 0, st>>>((double*)d_scratch, iters);   // warm-up
+  cudaEventRecord(e0, st);
+  k_probe_dfma<<<grid, threads, 0, st>>>((double*)d_scratch, iters);
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return Z4C_ECUDA;
+  *tflops_out = 2.0 * 8.0 * (double)iters * (double)grid * threads / ((double)ms * 1e-3) * 1e-12;
+  return Z4C_OK;
 }
 
 int z4c_sync(z4c_ctx* c) {

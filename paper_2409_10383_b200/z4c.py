@@ -20,7 +20,8 @@ LIB_PATH = os.path.join(_HERE, "libz4c.so")
 # every symbol include/z4c.h declares
 SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_initial_data", "z4c_step",
            "z4c_constraints", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
-           "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_time",
+           "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
+           "z4c_probe_fp64", "z4c_time",
            "z4c_last_error", "z4c_destroy"]
 
 
@@ -79,6 +80,8 @@ def load_library(path: Optional[str] = None):
     L.z4c_set_variant.argtypes = [vp, C.c_int]
     L.z4c_use_graph.argtypes = [vp, C.c_int]
     L.z4c_set_fused.argtypes = [vp, C.c_int]
+    L.z4c_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
+    L.z4c_probe_fp64.argtypes = [vp, vp, C.c_int, C.POINTER(C.c_double)]
     L.z4c_time.argtypes = [vp]
     L.z4c_time.restype = C.c_double
     L.z4c_last_error.argtypes = [vp]
@@ -87,7 +90,7 @@ def load_library(path: Optional[str] = None):
     L.z4c_destroy.restype = None
     for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_get_interior",
                "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
-               "z4c_set_fused"):
+               "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64"):
         getattr(L, fn).restype = C.c_int
     if path == LIB_PATH:
         _lib = L
@@ -215,6 +218,22 @@ class Z4c:
 
     def set_fused(self, enable: bool):
         self._check(self.lib.z4c_set_fused(self.h, int(bool(enable))))
+
+    def step_timed(self, nsteps: int = 1):
+        """z4c_step_timed: returns {"rhs": ms, "update": ms, "ghost": ms} summed over nsteps."""
+        ms = (C.c_double * 3)()
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_step_timed(self.h, int(nsteps), ms))
+        return {"rhs": ms[0], "update": ms[1], "ghost": ms[2]}
+
+    def probe_fp64(self, iters: int = 20000) -> float:
+        """z4c_probe_fp64: achieved DFMA TFLOP/s on this device."""
+        out = C.c_double()
+        with self.torch.cuda.device(self.device):
+            rc = self.lib.z4c_probe_fp64(self.stream.cuda_stream, self.work.data_ptr(), int(iters), C.byref(out))
+        if rc != 0:
+            raise Z4cError(rc, "z4c_probe_fp64 failed")
+        return float(out.value)
 
     def time(self) -> float:
         return float(self.lib.z4c_time(self.h))

@@ -25,7 +25,7 @@ def lib():
 def header_symbols():
     src = open(os.path.join(ROOT, "include", "z4c.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(z4c_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(z4c_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_symbols_all_exported(lib):
