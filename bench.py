@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py -- zone-cycles/s of the fp64 Z4c RK4 step (BASELINE.json `metric`).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+A "step" is one classical RK4 step (4 x [K2 RHS -> K3 stage update + enforcement + ghost push]) over the whole
+pack. Default workload: BASELINE.json configs[1], the linear gravitational wave on 64^3 cells in 64 blocks of
+16^3 (+3 ghosts). One JSON line is printed by rank 0. See DESIGN.md "Measurement" for every figure's definition.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from dataclasses import replace
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2409_10383_b200 import inputs as I  # noqa: E402
+
+# Algorithmic work per cell (flop census = oracle/z4c_oracle.cpp oz4c_count_flops,
+# add = mul = div = 1, no FMA fusion assumed; checked by tests/test_oracle_pins.py::test_flop_census).
+RHS_FLOPS_PER_CELL = 6034
+# doubles moved per cell and RK4 step by the O6 recurrence: 616, plus the ghost fill
+STEP_DOUBLES_PER_CELL = 616
+GHOST_DOUBLES_PER_GHOST_CELL_STEP = 4 * 22 * 2
+# K2 alone, per launch: reads y (22), writes P (22); stages 3-4 also read P (22)
+RHS_DOUBLES_PER_CELL = (44 + 44 + 66 + 66) / 4.0
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 DFMA/clk x 2 flop x max SM clock
+
+
+WORKLOAD_LABELS = {
+    "linear_wave_64": "configs[1]: linear wave 64^3 = 64 blocks of 16^3 (+3 ghosts), periodic",
+    "puncture_128": "configs[2]: single puncture 128^3 = 64 blocks of 32^3, outflow-copy",
+    "bbh_256": "configs[3]: two punctures 256^3 = 512 blocks of 32^3, outflow-copy",
+}
+
+
+def workload(name: str):
+    """(params, initial data, label). Inputs are synthetic and seeded."""
+    if name == "linear_wave_64":
+        p = I.params_linear_wave(64, 16)
+        return p, I.linear_wave_data(p), "configs[1]: linear wave 64^3 = 64 blocks of 16^3 (+3 ghosts), periodic"
+    if name == "puncture_128":
+        p, u, _ = I.config(2)
+        return p, u, "configs[2]: single puncture 128^3 = 64 blocks of 32^3, outflow-copy"
+    if name == "bbh_256":
+        p, u, _ = I.config(3)
+        return p, u, "configs[3]: two punctures 256^3 = 512 blocks of 32^3, outflow-copy"
+    if name.startswith("noise_"):            # configs[4] load sweep: noise_<n>_<nbx>x<nby>x<nbz>
+        _, n, lat = name.split("_")
+        nb = tuple(int(v) for v in lat.split("x"))
+        p = I.params_noise(int(n), nb, 0.1)
+        tile = tuple(2 if b % 2 == 0 else 1 for b in nb)
+        return p, I.tiled_noise_data(p, tile, 1000), f"configs[4]: noise, {nb} blocks of {n}^3, periodic"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+        self.period = period_s
+
+    def _once(self):
+        nv = self.nv
+        self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+        except Exception:
+            r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+                 0x4: "sw_power_cap", 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
+        for bit, nm in names.items():
+            if r & bit:
+                self.reasons.add(nm)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._once()
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr is not None:
+            self._stop.set()
+            self._thr.join()
+            if not self.samples:
+                try:
+                    self._once()
+                except Exception:
+                    pass
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def aggregate(local_ms: float, local_units: float, dist=None):
+    """Whole-job figures from per-rank ones: time = MAX over ranks, units = SUM over ranks
+    (replicas: no data-path collective). Works on gloo (CPU tensors) and nccl."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_units
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([local_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([local_units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(name: str):
+    """A bounded sample of the workload with identical per-cell arithmetic."""
+    if name == "linear_wave_64":
+        p = I.params_linear_wave(64, 16)
+        ps = replace(p, nb=(4, 1, 1))   # 64 x 16 x 16 periodic slab of the same wave
+        return ps, I.linear_wave_data(ps), "64x16x16 periodic slab of the 64^3 wave (same per-cell arithmetic)"
+    if name in ("puncture_128", "bbh_256"):
+        p, u, _ = I.config(2 if name == "puncture_128" else 3)
+        lo = p.N[0] // 2 - 16
+        ps = replace(p, n=32, nb=(1, 1, 1))
+        return ps, np.ascontiguousarray(u[:, lo:lo + 32, lo:lo + 32, lo:lo + 32]), "central 32^3 sub-box (clamped edges)"
+    p, u, _ = workload(name)
+    ps = replace(p, nb=(2, 1, 1))
+    return ps, I.noise_data(ps, 1000), f"2 blocks of {p.n}^3 of the noise pack"
+
+
+def time_oracle(name: str, steps: int, warmup: int, budget_s: float):
+    from oracle import oracle as O
+    O.build()
+    ps, us, what = oracle_sample(name)
+    us, _ = O.enforce(ps, us)
+    cores = O.num_threads()
+    t0 = time.perf_counter()
+    u1, _ = O.step(ps, us, 1)                      # calibration step (counts as warm-up)
+    t1 = time.perf_counter() - t0
+    for _ in range(max(0, warmup - 1)):
+        if (time.perf_counter() - t0) > budget_s * 0.25:
+            break
+        O.step(ps, us, 1)
+    k = max(1, min(steps, int(budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    O.step(ps, us, k)
+    dt = time.perf_counter() - t0
+    return {"zcps": ps.ncells * k / dt, "cores": cores, "steps": k, "ms_per_step": dt / k * 1e3,
+            "sample": f"{what}; {ps.ncells} cells x {k} RK4 steps"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    r = time_oracle(args.workload, args.steps, args.warmup, budget_s=60.0)
+    label = WORKLOAD_LABELS.get(args.workload, args.workload)
+    line = {"impl": "reference", "metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": r["zcps"],
+            "unit": "zone-cycles/s", "n_gpus": args.gpus, "steps": r["steps"], "warmup": args.warmup,
+            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": label, "impl": "CPU oracle (oracle/z4c_oracle.cpp, -O2 -ffp-contract=off, OpenMP)"},
+            "cpu_baseline": {"value": r["zcps"], "unit": "zone-cycles/s", "cores": r["cores"], "kind": "oracle",
+                             "sample": r["sample"]},
+            "e2e": {"value": r["zcps"], "unit": "zone-cycles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2409_10383_b200 import build, z4c
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the Z4c path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    build.build()
+    p, u0, label = workload(args.workload)
+    sim = z4c.Z4c(p, device=f"cuda:{local_rank}")
+    sim.set_variant(args.variant)
+    sim.set_fused(not args.no_fuse)
+    sim.use_graph(not args.no_graph)
+    K, W = args.steps, max(args.warmup, 3)
+    ncells = p.ncells
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput ---------------------------------------------------------
+    sim.set_initial_data(u0)
+    sim.step(W)
+    sim.sync()
+    l0 = sim.launch_count()
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    with torch.cuda.stream(sim.stream):
+        e0.record(sim.stream)
+        sim.step(K)
+        e1.record(sim.stream)
+    barrier()
+    clocks = sampler.stop()
+    ms_local = e0.elapsed_time(e1)
+    launches = sim.launch_count() - l0
+    sim.sync()                                            # raises if the device error flag is set
+    ms, units = aggregate(ms_local, float(ncells) * K, dist if world > 1 else None)
+    zcps = units / (ms * 1e-3)
+
+    # ---- per-kernel times over the same K steps (events between kernels, no graph) -------------
+    sim.step_timed(2)
+    kt = sim.step_timed(K)
+    rhs_ms = kt["rhs"] / (4 * K)
+    fp64_peak = sim.probe_fp64()
+    hbm_peak, hbm_src = measured_peaks()
+    rhs_tflops = RHS_FLOPS_PER_CELL * ncells / (rhs_ms * 1e-3) * 1e-12
+    rhs_gbs = RHS_DOUBLES_PER_CELL * 8 * ncells / (rhs_ms * 1e-3) * 1e-9
+    g = p.ng
+    ghost_cells = p.nblocks * ((p.n + 2 * g) ** 3 - p.n ** 3)
+    step_bytes = (STEP_DOUBLES_PER_CELL * ncells + GHOST_DOUBLES_PER_GHOST_CELL_STEP * ghost_cells) * 8
+    total_kt = kt["rhs"] + kt["update"] + kt["ghost"]
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ------
+    h_in = torch.from_numpy(u0).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    Ke = max(3, min(K, 20))
+    for _ in range(2):
+        sim.set_initial_data(h_in)
+        sim.step(1)
+        sim.get_interior(h_out.numpy())
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        sim.set_initial_data(h_in)            # H2D of the step's input (synchronises)
+        sim.step(1)
+        sim.get_interior(h_out.numpy())       # D2H of the step's result (synchronises)
+    barrier()
+    e2e_ms, e2e_units = aggregate((time.perf_counter() - t0) * 1e3, float(ncells) * Ke, dist if world > 1 else None)
+    nbytes = int(u0.nbytes)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        r = time_oracle(args.workload, 1000, 1, budget_s=15.0)
+        cpu = {"value": r["zcps"], "unit": "zone-cycles/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+
+    if rank == 0:
+        line = {
+            "metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": zcps, "unit": "zone-cycles/s", "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": label, "cells_per_gpu": ncells, "blocks": p.nblocks, "n": p.n, "ghosts": g,
+                       "parallelism": "replicas" if world > 1 else "1 GPU",
+                       "l2": "no flush: y+P+Q working set %.0f MB > 126 MB L2" %
+                             ((sim.state.numel() + sim.work.numel()) * 8 / 1e6),
+                       "graph": not args.no_graph, "fused_ghost_push": not args.no_fuse, "rhs_variant": args.variant},
+            "clocks": clocks,
+            "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": "zone-cycles/s", "h2d_bytes_per_step": nbytes,
+                    "d2h_bytes_per_step": nbytes, "steps": Ke,
+                    "what": "z4c_set_initial_data(host) + z4c_step(1) + z4c_get_interior(host) per step, pinned"},
+            "gpu_launches": int(launches),
+            "roofline": {"kernel": "K2 z4c_rhs", "bound": "alu", "achieved": rhs_tflops, "peak": fp64_peak,
+                         "unit": "TFLOP/s", "frac": rhs_tflops / fp64_peak, "traffic": None,
+                         "peak_source": "measured live: z4c_probe_fp64 DFMA loop (nominal %.1f at 1965 MHz)" % FP64_NOMINAL_TFLOPS,
+                         "flops_per_cell": RHS_FLOPS_PER_CELL, "ms_per_launch": rhs_ms,
+                         "hbm_gbs_algorithmic": rhs_gbs, "share_of_step": kt["rhs"] / total_kt},
+            "step_roofline": {"bound": "hbm", "achieved": step_bytes * K / (ms_local * 1e-3) * 1e-9, "peak": hbm_peak,
+                              "unit": "GB/s", "frac": step_bytes * K / (ms_local * 1e-3) * 1e-9 / hbm_peak,
+                              "peak_source": hbm_src, "bytes_per_cell_step": step_bytes / ncells,
+                              "kernel_ms_per_step": {k: v / K for k, v in kt.items()}},
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="linear_wave_64")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-fuse", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
