@@ -35,6 +35,8 @@ struct z4c_ctx {
   int fuse_ghosts;
   cudaGraphExec_t graph_exec;
   int graph_launches;
+  CUtensorMap ymap;   // TMA descriptor of the state pack (tuned K2)
+  int have_ymap;
   std::string err;
 };
 
@@ -102,8 +104,9 @@ int launch_ghost_fill(z4c_ctx* c) {
 
 int launch_rhs(z4c_ctx* c, double coef, double dt) {
   const Pack& g = c->g;
-  if (c->variant == 0 && rhs_tiled_supported(g)) {
-    launch_rhs_tiled(g, c->y, c->P, c->fd, c->sp, coef, dt, c->stream);
+  if (c->variant == 0 && c->have_ymap) {
+    cudaError_t e = launch_rhs_tiled_t<RhsTile>(c->ymap, g, c->P, c->fd, c->sp, coef, dt, c->stream);
+    if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
     return check_launch(c, "k_rhs_tiled");
   }
   const int tx = (g.n + K2_TX - 1) / K2_TX, ty = (g.n + K2_TY - 1) / K2_TY, tz = (g.n + K2_TZ - 1) / K2_TZ;
@@ -267,6 +270,7 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->fuse_ghosts = 1;
   c->graph_exec = nullptr;
   c->graph_launches = 0;
+  c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->y, &c->ymap) ? 1 : 0;
   cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
   if (e != cudaSuccess) {
     delete c;

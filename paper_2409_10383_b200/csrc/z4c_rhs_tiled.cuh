@@ -1,7 +1,238 @@
-// placeholder, replaced below
+// K2, tuned variant: the RHS kernel with TMA-staged shared-memory tiles (sm_100a).
+//
+// One CTA of TX*TY*TZ threads owns a TX x TY x TZ tile of interior cells of one MeshBlock, one cell per
+// thread. The 22 fields are streamed through a ring of NSTAGE shared-memory buffers, one (TX+6)(TY+6)(TZ+6)
+// halo tile per field, each fetched by a single 5-D TMA box copy (cp.async.bulk.tensor, fp64 elements,
+// coordinates (i, j, k, block, field) of the state pack) that completes on an mbarrier. While the threads take
+// the stencils of field f out of shared memory -- centred 1st/2nd derivatives, upwinded advection and
+// Kreiss-Oliger dissipation (S2 of SURVEY.md 8(a)) -- the copy engine is already fetching fields f+1..f+NSTAGE-1,
+// so no thread ever waits on a global-memory load. The Z4c sources (S3) then run in registers.
+//
+// Upwinding without selects: with e_s = u_{+s} - u_{-s} and the Kreiss-Oliger sum ko = s3 - 6 s2 + 15 s1,
+//   D^+ + D^- = (e3 - 6 e2 + 21 e1)/(12h),   D^+ - D^- = ko/(12h)
+// hence beta D^{sign(beta)} u = [ beta (e3 - 6 e2 + 21 e1) + |beta| ko ] / (24h): the 7 values loaded for the
+// KO operator serve the advection term too, with no per-axis branch or select (O3, reading Q9).
 #pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
 #include "z4c_kernels.cuh"
+
 namespace z4c {
-inline bool rhs_tiled_supported(const Pack&) { return false; }
-inline void launch_rhs_tiled(const Pack&, const double*, double*, const FdConst&, const SrcParams&, double, double, cudaStream_t) {}
+
+// ---- mbarrier / TMA primitives (PTX) ------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+__device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1,
+                                            int c2, int c3, int c4) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+      : "memory");
+}
+
+// ---- tile geometry ---------------------------------------------------------------------------------
+template <int TX_, int TY_, int TZ_, int NSTAGE_>
+struct TileCfg {
+  static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NSTAGE = NSTAGE_;
+  static constexpr int THREADS = TX * TY * TZ;
+  static constexpr int HX = TX + 2 * NG, HY = TY + 2 * NG, HZ = TZ + 2 * NG;
+  static constexpr int SY = HX, SZ = HX * HY;          // element strides inside the halo tile
+  static constexpr int TILE_ELEMS = HX * HY * HZ;
+  static constexpr int TILE_BYTES = TILE_ELEMS * 8;
+  static constexpr int STAGE_BYTES = (TILE_BYTES + 127) / 128 * 128;
+  static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 128;
+};
+
+// field streaming order: the shift first (its sign and size weight every other field's advection)
+__host__ __device__ constexpr int stream_field(int it) { return it < 3 ? BETAX + it : it - 3; }
+
+// One axis of one field out of the shared-memory tile. t points at the cell, S is the compile-time stride.
+template <int S, bool WANT_D1, bool WANT_D2>
+__device__ __forceinline__ void axis_tile(const double* t, const double c, const double bw, const double aw,
+                                          const FdConst& fd, double& d1, double& d2, double& adv, double& ko) {
+  const double lm3 = t[-3 * S], lm2 = t[-2 * S], lm1 = t[-S], lp1 = t[S], lp2 = t[2 * S], lp3 = t[3 * S];
+  const double e1 = lp1 - lm1, e2 = lp2 - lm2, e3 = lp3 - lm3;
+  const double s1 = (lp1 - c) + (lm1 - c), s2 = (lp2 - c) + (lm2 - c), s3 = (lp3 - c) + (lm3 - c);
+  if (WANT_D1) d1 = (8.0 * e1 - e2) * fd.inv12h;
+  if (WANT_D2) d2 = (16.0 * s1 - s2) * fd.inv12h2;
+  const double k = s3 - 6.0 * s2 + 15.0 * s1;
+  const double sy = e3 - 6.0 * e2 + 21.0 * e1;
+  adv += bw * sy + aw * k;
+  ko += k;
+}
+
+// mixed second derivative from the tile, compile-time strides
+template <int SA, int SB>
+__device__ __forceinline__ double mixed_tile(const double* t) {
+  auto inner = [&](const double* q) { return 8.0 * (q[SA] - q[-SA]) - (q[2 * SA] - q[-2 * SA]); };
+  return 8.0 * (inner(t + SB) - inner(t - SB)) - (inner(t + 2 * SB) - inner(t - 2 * SB));
+}
+
+template <class Cfg, int F>
+__device__ __forceinline__ void field_from_tile(const double* t, const double* bw, const double* aw,
+                                                const FdConst& fd, const SrcParams& sp, double* u, Derivs& D,
+                                                double* out) {
+  constexpr bool W1 = need_d1(F), W2 = need_d2(F);
+  const double c = t[0];
+  u[F] = c;
+  double adv = 0.0, ko = 0.0, d1x = 0, d1y = 0, d1z = 0, d2x = 0, d2y = 0, d2z = 0;
+  axis_tile<1, W1, W2>(t, c, bw[0], aw[0], fd, d1x, d2x, adv, ko);
+  axis_tile<Cfg::SY, W1, W2>(t, c, bw[1], aw[1], fd, d1y, d2y, adv, ko);
+  axis_tile<Cfg::SZ, W1, W2>(t, c, bw[2], aw[2], fd, d1z, d2z, adv, ko);
+  if (W1) { D.d1[F][0] = d1x; D.d1[F][1] = d1y; D.d1[F][2] = d1z; }
+  if (W2) {
+    D.d2[F][sym(0, 0)] = d2x; D.d2[F][sym(1, 1)] = d2y; D.d2[F][sym(2, 2)] = d2z;
+    D.d2[F][sym(0, 1)] = mixed_tile<1, Cfg::SY>(t) * fd.inv144h2;
+    D.d2[F][sym(0, 2)] = mixed_tile<1, Cfg::SZ>(t) * fd.inv144h2;
+    D.d2[F][sym(1, 2)] = mixed_tile<Cfg::SY, Cfg::SZ>(t) * fd.inv144h2;
+  }
+  const double cadv = (F == ALPHA) ? sp.lapse_advect : (F >= BETAX ? sp.shift_advect : 1.0);
+  out[F] = cadv * adv + ko * fd.ko;
+}
+
+template <class Cfg, int IT>
+struct FieldLoop {
+  __device__ __forceinline__ static void run(const CUtensorMap* map, unsigned char* tiles, uint64_t* full,
+                                             const int toff, const int cx, const int cy, const int cz, const int b,
+                                             const bool active, double* bw, double* aw, const FdConst& fd,
+                                             const SrcParams& sp, double* u, Derivs& D, double* out) {
+    constexpr int S = IT % Cfg::NSTAGE;
+    constexpr int F = stream_field(IT);
+    if (IT >= 3) mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);   // the first three were waited for up front
+    const double* t = reinterpret_cast<const double*>(tiles + S * Cfg::STAGE_BYTES) + toff;
+    if (active) field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out);
+    if (IT + Cfg::NSTAGE < NF) {
+      __syncthreads();   // every thread is done reading stage S
+      if (threadIdx.x == 0) {
+        mbar_expect_tx(&full[S], Cfg::TILE_BYTES);
+        tma_load_5d(tiles + S * Cfg::STAGE_BYTES, map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
+      }
+    }
+    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
+  }
+};
+template <class Cfg>
+struct FieldLoop<Cfg, NF> {
+  __device__ __forceinline__ static void run(const CUtensorMap*, unsigned char*, uint64_t*, int, int, int, int, int,
+                                             bool, double*, double*, const FdConst&, const SrcParams&, double*,
+                                             Derivs&, double*) {}
+};
+
+template <class Cfg>
+__global__ void __launch_bounds__(Cfg::THREADS, 1)
+    k_rhs_tiled(const __grid_constant__ CUtensorMap map, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
+                double c, double dt, int tiles_x, int tiles_y, int tiles_z) {
+  static_assert(Cfg::NSTAGE >= 3, "the three shift components are staged together");
+  extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
+  uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::NSTAGE * Cfg::STAGE_BYTES);
+  const int tid = threadIdx.x;
+  const int lx = tid % Cfg::TX, ly = (tid / Cfg::TX) % Cfg::TY, lz = tid / (Cfg::TX * Cfg::TY);
+  int t = blockIdx.x;
+  const int tx = t % tiles_x; t /= tiles_x;
+  const int ty = t % tiles_y; t /= tiles_y;
+  const int tz = t % tiles_z; t /= tiles_z;
+  const int b = t;
+  // padded coordinates of the halo tile's origin = interior coordinates of the tile's first cell
+  const int cx = tx * Cfg::TX, cy = ty * Cfg::TY, cz = tz * Cfg::TZ;
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < Cfg::NSTAGE; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < Cfg::NSTAGE; ++s) {
+      mbar_expect_tx(&full[s], Cfg::TILE_BYTES);
+      tma_load_5d(tiles + s * Cfg::STAGE_BYTES, &map, &full[s], cx, cy, cz, b, stream_field(s));
+    }
+  }
+  const int toff = (lz + NG) * Cfg::SZ + (ly + NG) * Cfg::SY + lx + NG;
+  const int i = cx + lx, j = cy + ly, k = cz + lz;
+  const bool active = i < g.n && j < g.n && k < g.n;
+  double bw[3], aw[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    mbar_wait(&full[a], 0);
+    const double beta = reinterpret_cast<const double*>(tiles + a * Cfg::STAGE_BYTES)[toff];
+    bw[a] = beta * (0.5 * fd.inv12h);
+    aw[a] = fabs(beta) * (0.5 * fd.inv12h);
+  }
+  double u[NF], out[NF];
+  Derivs D;
+  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
+  if (!active) return;
+  z4c_sources(sp, u, D, out);
+  double* pc = Preg + (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
+  if (c != 0.0) {
+#pragma unroll
+    for (int f = 0; f < NF; ++f) pc[f * g.is] = c * pc[f * g.is] + dt * out[f];
+  } else {
+#pragma unroll
+    for (int f = 0; f < NF; ++f) pc[f * g.is] = dt * out[f];
+  }
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+using RhsTile = TileCfg<16, 4, 4, 3>;
+
+inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
+
+// Encode the 5-D tensor map (i, j, k, block, field) of the state pack with a halo-tile box. Returns false if
+// the driver entry point is unavailable or rejects the geometry (the caller then keeps the plain variant).
+template <class Cfg>
+inline bool make_state_tensor_map(const Pack& g, const double* y, CUtensorMap* out) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                               const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                               CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess)
+    return false;
+  const cuuint64_t m = (cuuint64_t)g.m;
+  const cuuint64_t dims[5] = {m, m, m, (cuuint64_t)g.nblk, (cuuint64_t)NF};
+  const cuuint64_t strides[4] = {m * 8, m * m * 8, m * m * m * 8, (cuuint64_t)g.fs * 8};
+  const cuuint32_t box[5] = {(cuuint32_t)Cfg::HX, (cuuint32_t)Cfg::HY, (cuuint32_t)Cfg::HZ, 1, 1};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  const CUresult r = ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)y, dims, strides, box, estr,
+                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+template <class Cfg>
+inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const Pack& g, double* P, const FdConst& fd,
+                                      const SrcParams& sp, double coef, double dt, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
+  const long long nblocks = (long long)tx * ty * tz * g.nblk;
+  if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+  k_rhs_tiled<Cfg><<<(unsigned)nblocks, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(map, g, P, fd, sp, coef, dt, tx, ty, tz);
+  return cudaSuccess;
+}
+
+}  // namespace z4c
