@@ -36,6 +36,7 @@ struct z4c_ctx {
   cudaGraphExec_t graph_exec;
   int graph_launches;
   CUtensorMap ymap;   // TMA descriptor of the state pack (tuned K2)
+  CUtensorMap ymapB;  // same with the 16x4x2 tile box (experimental variants 2, 3)
   int have_ymap;
   std::string err;
 };
@@ -104,6 +105,13 @@ int launch_ghost_fill(z4c_ctx* c) {
 
 int launch_rhs(z4c_ctx* c, double coef, double dt) {
   const Pack& g = c->g;
+  if ((c->variant == 2 || c->variant == 3) && c->have_ymap) {
+    cudaError_t e = c->variant == 2
+        ? launch_rhs_tiled_t<RhsTileB>(c->ymapB, g, c->P, c->fd, c->sp, coef, dt, c->stream)
+        : launch_rhs_tiled_t<RhsTileC>(c->ymapB, g, c->P, c->fd, c->sp, coef, dt, c->stream);
+    if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
+    return check_launch(c, "k_rhs_tiled");
+  }
   if (c->variant == 0 && c->have_ymap) {
     cudaError_t e = launch_rhs_tiled_t<RhsTile>(c->ymap, g, c->P, c->fd, c->sp, coef, dt, c->stream);
     if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
@@ -270,7 +278,8 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->fuse_ghosts = 1;
   c->graph_exec = nullptr;
   c->graph_launches = 0;
-  c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->y, &c->ymap) ? 1 : 0;
+  c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->y, &c->ymap) &&
+                 make_state_tensor_map<RhsTileB>(c->g, c->y, &c->ymapB) ? 1 : 0;
   cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
   if (e != cudaSuccess) {
     delete c;
@@ -442,7 +451,7 @@ int z4c_sync(z4c_ctx* c) {
 int64_t z4c_launch_count(const z4c_ctx* c) { return c ? c->launches : 0; }
 
 int z4c_set_variant(z4c_ctx* c, int variant) {
-  if (!c || variant < 0 || variant > 1) return Z4C_EINVAL;
+  if (!c || variant < 0 || variant > 3) return Z4C_EINVAL;
   if (variant != c->variant) drop_graph(c);
   c->variant = variant;
   return Z4C_OK;

@@ -49,9 +49,9 @@ __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* m
 }
 
 // ---- tile geometry ---------------------------------------------------------------------------------
-template <int TX_, int TY_, int TZ_, int NSTAGE_>
+template <int TX_, int TY_, int TZ_, int NSTAGE_, int MINB_ = 1>
 struct TileCfg {
-  static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NSTAGE = NSTAGE_;
+  static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NSTAGE = NSTAGE_, MINB = MINB_;
   static constexpr int THREADS = TX * TY * TZ;
   static constexpr int HX = TX + 2 * NG, HY = TY + 2 * NG, HZ = TZ + 2 * NG;
   static constexpr int SY = HX, SZ = HX * HY;          // element strides inside the halo tile
@@ -137,7 +137,7 @@ struct FieldLoop<Cfg, NF> {
 };
 
 template <class Cfg>
-__global__ void __launch_bounds__(Cfg::THREADS, 1)
+__global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     k_rhs_tiled(const __grid_constant__ CUtensorMap map, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
                 double c, double dt, int tiles_x, int tiles_y, int tiles_z) {
   static_assert(Cfg::NSTAGE >= 3, "the three shift components are staged together");
@@ -192,7 +192,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1)
 }
 
 // ---- host side -------------------------------------------------------------------------------------
-using RhsTile = TileCfg<16, 4, 4, 3>;
+using RhsTile = TileCfg<16, 4, 4, 3>;        // 256 threads, 255 registers, 1 CTA/SM
+using RhsTileB = TileCfg<16, 4, 2, 3, 3>;    // 128 threads, <=168 registers, 3 CTAs/SM
+using RhsTileC = TileCfg<16, 4, 2, 3, 4>;    // 128 threads, <=128 registers, 4 CTAs/SM
 
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 
