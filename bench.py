@@ -221,7 +221,7 @@ def run_ours(args):
     p, u0, label = workload(args.workload)
     sim = z4c.Z4c(p, device=f"cuda:{local_rank}")
     sim.set_variant(args.variant)
-    sim.set_fused(not args.no_fuse)
+    sim.set_fused(args.fuse)
     sim.use_graph(not args.no_graph)
     K, W = args.steps, max(args.warmup, 3)
     ncells = p.ncells
@@ -297,7 +297,7 @@ def run_ours(args):
                        "parallelism": "replicas" if world > 1 else "1 GPU",
                        "l2": "no flush: y+P+Q working set %.0f MB > 126 MB L2" %
                              ((sim.state.numel() + sim.work.numel()) * 8 / 1e6),
-                       "graph": not args.no_graph, "fused_ghost_push": not args.no_fuse, "rhs_variant": args.variant},
+                       "graph": not args.no_graph, "fuse_mode": args.fuse, "rhs_variant": args.variant},
             "clocks": clocks,
             "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": "zone-cycles/s", "h2d_bytes_per_step": nbytes,
                     "d2h_bytes_per_step": nbytes, "steps": Ke,
@@ -329,7 +329,7 @@ def main():
     ap.add_argument("--workload", default="linear_wave_64")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-graph", action="store_true")
-    ap.add_argument("--no-fuse", action="store_true")
+    ap.add_argument("--fuse", type=int, default=2, help="0: K2,K3,K1; 1: K2,K3+push; 2: one kernel per RK stage")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -73,7 +73,8 @@ typedef struct {
 /* Bytes of the state buffer y: 22*N_b*m^3*8. Returns 0 if the parameters are invalid. */
 size_t z4c_state_bytes(const z4c_params* p);
 
-/* Bytes of the workspace (RK registers P and Q on interior cells, reduction scratch, error flag).
+/* Bytes of the workspace (RK registers P and Q on interior cells, reduction scratch, error flag, and the
+ * second state buffer of the one-kernel-per-stage mode: about 2*22*N_b*n^3*8 + 22*N_b*m^3*8).
  * Returns 0 if the parameters are invalid. */
 size_t z4c_workspace_bytes(const z4c_params* p);
 
@@ -134,16 +135,21 @@ int z4c_sync(z4c_ctx* ctx);
 
 /* Number of kernel launches the library has enqueued on this context so far. */
 int64_t z4c_launch_count(const z4c_ctx* ctx);
-/* Select the RHS kernel variant (0 = default tuned kernel, 1 = plain global-memory kernel).
- * For A/B measurements; both variants compute the same values. */
+/* Select the RHS kernel variant: 0 = tuned kernel, TMA-staged 16x4x4 tiles, 256 threads (default);
+ * 1 = plain global-memory kernel; 2 = tuned kernel with 16x4x2 tiles, 128 threads, 2 CTAs per SM.
+ * For A/B measurements; all variants compute the same values. */
 int z4c_set_variant(z4c_ctx* ctx, int variant);
 /* Enable (1) / disable (0) CUDA-graph replay of the RK4 step inside z4c_step. Default 0. */
 int z4c_use_graph(z4c_ctx* ctx, int enable);
 
-/* Fuse the ghost fill into the stage update ("ghost push": the thread that updates an interior cell also
- * writes that cell's ghost images in the neighbouring blocks; same values as K1, one pass less over the
- * state). 1 = fused (default), 0 = separate K3 and K1 launches. */
-int z4c_set_fused(z4c_ctx* ctx, int enable);
+/* How much of an RK stage runs in one kernel. mode 0: three launches per stage, K2 -> K3 -> K1.
+ * mode 1: K2 -> K3 with "ghost push" (the thread that updates an interior cell also writes that cell's ghost
+ * images in the neighbouring blocks; same values as K1, one pass less over the state).
+ * mode 2 (default): ONE launch per stage -- the tuned K2 applies the RK recurrence, the enforcement and the
+ * ghost push to each cell while its values are still in registers, reading the state from one buffer and
+ * writing the next one to a second buffer kept in the workspace (4 stages: the caller's buffer is current
+ * again at the end of every step). Falls back to mode 1 where the tuned K2 is unavailable (odd n, variant 1). */
+int z4c_set_fused(z4c_ctx* ctx, int mode);
 
 double z4c_time(const z4c_ctx* ctx);             /* simulation time = steps taken * dt */
 const char* z4c_last_error(const z4c_ctx* ctx);  /* host string owned by the context ("" if none) */

@@ -35,8 +35,9 @@ struct z4c_ctx {
   int fuse_ghosts;
   cudaGraphExec_t graph_exec;
   int graph_launches;
-  CUtensorMap ymap;   // TMA descriptor of the state pack (tuned K2)
-  CUtensorMap ymapB;  // same with the 16x4x2 tile box (experimental variants 2, 3)
+  double* ybuf[2];    // ybuf[0] = y (caller's state), ybuf[1] = second state buffer in the workspace
+  CUtensorMap ymap[2];  // TMA descriptors of the two state buffers (tuned K2)
+  CUtensorMap ymap2[2]; // same with the 128-thread tile box
   int have_ymap;
   std::string err;
 };
@@ -105,15 +106,8 @@ int launch_ghost_fill(z4c_ctx* c) {
 
 int launch_rhs(z4c_ctx* c, double coef, double dt) {
   const Pack& g = c->g;
-  if ((c->variant == 2 || c->variant == 3) && c->have_ymap) {
-    cudaError_t e = c->variant == 2
-        ? launch_rhs_tiled_t<RhsTileB>(c->ymapB, g, c->P, c->fd, c->sp, coef, dt, c->stream)
-        : launch_rhs_tiled_t<RhsTileC>(c->ymapB, g, c->P, c->fd, c->sp, coef, dt, c->stream);
-    if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
-    return check_launch(c, "k_rhs_tiled");
-  }
-  if (c->variant == 0 && c->have_ymap) {
-    cudaError_t e = launch_rhs_tiled_t<RhsTile>(c->ymap, g, c->P, c->fd, c->sp, coef, dt, c->stream);
+  if (c->variant != 1 && c->have_ymap) {
+    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{});
     if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
     return check_launch(c, "k_rhs_tiled");
   }
@@ -145,10 +139,37 @@ int launch_stage_update(z4c_ctx* c, int stage, bool push) {
   return check_launch(c, "k_stage_update");
 }
 
+// One RK stage as ONE kernel: RHS from ybuf[in] (TMA tiles), recurrence + enforcement in registers, updated
+// state and its ghost images written to ybuf[1-in].
+template <class Cfg>
+cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, int stage, const StageArgs& sa) {
+  switch (stage) {
+    case 1: return launch_rhs_tiled_t<Cfg, 1>(map, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
+    case 2: return launch_rhs_tiled_t<Cfg, 2>(map, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
+    case 3: return launch_rhs_tiled_t<Cfg, 3>(map, c->g, c->P, c->fd, c->sp, -0.5, c->dt, c->stream, sa);
+    default: return launch_rhs_tiled_t<Cfg, 4>(map, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa);
+  }
+}
+int launch_fused_stage(z4c_ctx* c, int stage, int in) {
+  StageArgs sa{c->Q, c->ybuf[1 - in], c->prm.chi_floor, c->flag};
+  cudaError_t e = c->variant == 2 ? launch_fused_stage_t<RhsTile2>(c, c->ymap2[in], stage, sa)
+                                  : launch_fused_stage_t<RhsTile>(c, c->ymap[in], stage, sa);
+  if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
+  return check_launch(c, "k_rhs_tiled<stage>");
+}
+bool fully_fused(const z4c_ctx* c) { return c->fuse_ghosts == 2 && c->variant != 1 && c->have_ymap; }
+
 // One classical RK4 step in the 3-register recurrence: per stage
 // K2 (P <- c_s P + dt L(y)) -> K3 (update + enforcement) -> K1 (ghost fill).
 int enqueue_step(z4c_ctx* c) {
   static const double coef[4] = {0.0, 0.0, -0.5, 2.0};
+  if (fully_fused(c)) {   // 4 launches; the state ping-pongs y -> y2 -> y -> y2 -> y
+    for (int s = 1; s <= 4; ++s) {
+      int rc = launch_fused_stage(c, s, (s - 1) & 1);
+      if (rc) return rc;
+    }
+    return Z4C_OK;
+  }
   for (int s = 1; s <= 4; ++s) {
     int rc = launch_rhs(c, coef[s - 1], c->dt);
     if (rc) return rc;
@@ -170,7 +191,13 @@ int enqueue_step_timed(z4c_ctx* c, cudaEvent_t* ev, double* ms) {
   int kind[16];
   int rc = check_cuda(c, cudaEventRecord(ev[ne++], c->stream), "event record");
   if (rc) return rc;
-  for (int s = 1; s <= 4; ++s) {
+  for (int s = 1; s <= 4 && fully_fused(c); ++s) {
+    rc = launch_fused_stage(c, s, (s - 1) & 1);
+    if (rc) return rc;
+    kind[ne] = 0;
+    cudaEventRecord(ev[ne++], c->stream);
+  }
+  for (int s = 1; s <= 4 && !fully_fused(c); ++s) {
     rc = launch_rhs(c, coef[s - 1], c->dt);
     if (rc) return rc;
     kind[ne] = 0;
@@ -241,7 +268,8 @@ size_t z4c_workspace_bytes(const z4c_params* p) {
   if (!valid_params(p)) return 0;
   const Pack g = make_pack(*p);
   const size_t reg = align_up((size_t)NF * (size_t)g.is * sizeof(double));
-  return 2 * reg + align_up((size_t)K4_MAX_PARTS * 8 * sizeof(double)) + align_up(8 * sizeof(double)) + ALIGN;
+  return 2 * reg + align_up((size_t)K4_MAX_PARTS * 8 * sizeof(double)) + align_up(8 * sizeof(double)) + ALIGN +
+         align_up((size_t)NF * (size_t)g.fs * sizeof(double));
 }
 
 int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stream, z4c_ctx** out) {
@@ -270,16 +298,20 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->partial = (double*)(w + 2 * reg);
   c->result = (double*)(w + 2 * reg + align_up((size_t)K4_MAX_PARTS * 8 * sizeof(double)));
   c->flag = (int*)((char*)c->result + align_up(8 * sizeof(double)));
+  c->ybuf[0] = c->y;
+  c->ybuf[1] = (double*)((char*)c->flag + ALIGN);
   c->stream = (cudaStream_t)cuda_stream;
   c->steps = 0;
   c->launches = 0;
   c->variant = 0;
   c->use_graph = 0;
-  c->fuse_ghosts = 1;
+  c->fuse_ghosts = 2;
   c->graph_exec = nullptr;
   c->graph_launches = 0;
-  c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->y, &c->ymap) &&
-                 make_state_tensor_map<RhsTileB>(c->g, c->y, &c->ymapB) ? 1 : 0;
+  c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->ybuf[0], &c->ymap[0]) &&
+                 make_state_tensor_map<RhsTile>(c->g, c->ybuf[1], &c->ymap[1]) &&
+                 make_state_tensor_map<RhsTile2>(c->g, c->ybuf[0], &c->ymap2[0]) &&
+                 make_state_tensor_map<RhsTile2>(c->g, c->ybuf[1], &c->ymap2[1]) ? 1 : 0;
   cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
   if (e != cudaSuccess) {
     delete c;
@@ -401,7 +433,7 @@ int z4c_eval_rhs(z4c_ctx* c, double* d_out) {
 
 int z4c_enforce(z4c_ctx* c) {
   if (!c) return Z4C_EINVAL;
-  if (c->fuse_ghosts) return launch_stage_update(c, 0, true);
+  if (c->fuse_ghosts) return launch_stage_update(c, 0, true);  // K3 with ghost push
   int rc = launch_stage_update(c, 0, false);
   if (rc) return rc;
   return launch_ghost_fill(c);
@@ -451,7 +483,7 @@ int z4c_sync(z4c_ctx* c) {
 int64_t z4c_launch_count(const z4c_ctx* c) { return c ? c->launches : 0; }
 
 int z4c_set_variant(z4c_ctx* c, int variant) {
-  if (!c || variant < 0 || variant > 3) return Z4C_EINVAL;
+  if (!c || variant < 0 || variant > 2) return Z4C_EINVAL;
   if (variant != c->variant) drop_graph(c);
   c->variant = variant;
   return Z4C_OK;
@@ -466,8 +498,9 @@ int z4c_use_graph(z4c_ctx* c, int enable) {
 
 int z4c_set_fused(z4c_ctx* c, int enable) {
   if (!c) return Z4C_EINVAL;
-  if ((enable ? 1 : 0) != c->fuse_ghosts) drop_graph(c);
-  c->fuse_ghosts = enable ? 1 : 0;
+  if (enable < 0 || enable > 2) return Z4C_EINVAL;
+  if (enable != c->fuse_ghosts) drop_graph(c);
+  c->fuse_ghosts = enable;
   return Z4C_OK;
 }
 

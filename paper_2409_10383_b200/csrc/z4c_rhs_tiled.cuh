@@ -136,10 +136,23 @@ struct FieldLoop<Cfg, NF> {
                                              Derivs&, double*) {}
 };
 
-template <class Cfg>
+// Arguments of the fused stage epilogue (STAGE 1..4): the RK registers, the OTHER state buffer (the stage
+// reads y_in through the tensor map and writes the updated, enforced state and its ghost images to y_out, so
+// no CTA ever reads a cell another CTA is writing), the chi floor and the error flag.
+struct StageArgs {
+  double* Q;
+  double* y_out;
+  double chi_floor;
+  int* flag;
+};
+
+// STAGE 0: P <- c*P + dt*(F(y) + Q_KO(y)) only (z4c_eval_rhs and the unfused path).
+// STAGE 1..4: K2 + K3 + K1 in one pass ("one kernel per RK stage"): the same recurrence and the same
+// expression forms as k_stage_update, applied to the cell while its 22 values are still in registers.
+template <class Cfg, int STAGE>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     k_rhs_tiled(const __grid_constant__ CUtensorMap map, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
-                double c, double dt, int tiles_x, int tiles_y, int tiles_z) {
+                double c, double dt, int tiles_x, int tiles_y, int tiles_z, StageArgs sa) {
   static_assert(Cfg::NSTAGE >= 3, "the three shift components are staged together");
   extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
   uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::NSTAGE * Cfg::STAGE_BYTES);
@@ -181,20 +194,75 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
   if (!active) return;
   z4c_sources(sp, u, D, out);
-  double* pc = Preg + (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
-  if (c != 0.0) {
+  const long long ci = (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
+  double* pc = Preg + ci;
+  if (STAGE == 0) {
+    if (c != 0.0) {
 #pragma unroll
-    for (int f = 0; f < NF; ++f) pc[f * g.is] = c * pc[f * g.is] + dt * out[f];
-  } else {
+      for (int f = 0; f < NF; ++f) pc[f * g.is] = c * pc[f * g.is] + dt * out[f];
+    } else {
 #pragma unroll
-    for (int f = 0; f < NF; ++f) pc[f * g.is] = dt * out[f];
+      for (int f = 0; f < NF; ++f) pc[f * g.is] = dt * out[f];
+    }
+    return;
+  }
+  double* qc = sa.Q + ci;
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    if (STAGE == 1) {
+      const double P = dt * out[f];
+      qc[f * g.is] = P;
+      u[f] = u[f] + 0.5 * P;
+    } else if (STAGE == 2) {
+      const double P = dt * out[f];
+      const double Q = qc[f * g.is];
+      pc[f * g.is] = P;
+      u[f] = u[f] + 0.5 * (P - Q);
+      qc[f * g.is] = Q / 6.0;
+    } else if (STAGE == 3) {
+      const double P = -0.5 * pc[f * g.is] + dt * out[f];
+      const double Q = qc[f * g.is];
+      pc[f * g.is] = P;
+      u[f] = u[f] + P;
+      qc[f * g.is] = Q - P;
+    } else {
+      const double P = 2.0 * pc[f * g.is] + dt * out[f];
+      const double Q = qc[f * g.is];
+      u[f] = u[f] + (Q + P / 6.0);
+    }
+  }
+  bool bad = enforce_cell(u, sa.chi_floor);
+  bad |= any_nonfinite(u);
+  if (bad) *sa.flag = 1;
+  double* yo = sa.y_out + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
+#pragma unroll
+  for (int f = 0; f < NF; ++f) yo[f * g.fs] = u[f];
+  const bool edge = i < NG || i >= g.n - NG || j < NG || j >= g.n - NG || k < NG || k >= g.n - NG;
+  if (edge) {
+    int bx, by, bz;
+    block_coords(g, b, bx, by, bz);
+    int tbx[4], tlx[4], tby[4], tly[4], tbz[4], tlz[4];
+    const int ncx = push_targets(i, bx, g.n, g.nb[0], g.bc, tbx, tlx);
+    const int ncy = push_targets(j, by, g.n, g.nb[1], g.bc, tby, tly);
+    const int ncz = push_targets(k, bz, g.n, g.nb[2], g.bc, tbz, tlz);
+    for (int a = 0; a < ncz; ++a)
+      for (int bb = 0; bb < ncy; ++bb)
+        for (int cc = 0; cc < ncx; ++cc) {
+          if (a + bb + cc == 0) continue;
+          const long long tb = ((long long)tbz[a] * g.nb[1] + tby[bb]) * g.nb[0] + tbx[cc];
+          double* d = sa.y_out + tb * g.m3 + ((long long)tlz[a] * g.m + tly[bb]) * g.m + tlx[cc];
+#pragma unroll
+          for (int f = 0; f < NF; ++f) d[f * g.fs] = u[f];
+        }
   }
 }
 
 // ---- host side -------------------------------------------------------------------------------------
-using RhsTile = TileCfg<16, 4, 4, 3>;        // 256 threads, 255 registers, 1 CTA/SM
-using RhsTileB = TileCfg<16, 4, 2, 3, 3>;    // 128 threads, <=168 registers, 3 CTAs/SM
-using RhsTileC = TileCfg<16, 4, 2, 3, 4>;    // 128 threads, <=128 registers, 4 CTAs/SM
+// 256 threads, 255 registers, 1 CTA/SM. (Measured on 64^3: 128-thread tiles capped at 168 / 128 registers for
+// 3 / 4 CTAs per SM were slower, 0.183 / 0.219 ms against 0.170 ms per launch: the spills cost more than the
+// extra warps hide.)
+using RhsTile = TileCfg<16, 4, 4, 3>;
+using RhsTile2 = TileCfg<16, 4, 2, 3, 2>;   // 128 threads, 2 CTAs/SM: one CTA's epilogue overlaps the other's stencils
 
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 
@@ -221,19 +289,22 @@ inline bool make_state_tensor_map(const Pack& g, const double* y, CUtensorMap* o
   return r == CUDA_SUCCESS;
 }
 
-template <class Cfg>
+template <class Cfg, int STAGE>
 inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const Pack& g, double* P, const FdConst& fd,
-                                      const SrcParams& sp, double coef, double dt, cudaStream_t st) {
+                                      const SrcParams& sp, double coef, double dt, cudaStream_t st,
+                                      const StageArgs& sa) {
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         Cfg::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
   const long long nblocks = (long long)tx * ty * tz * g.nblk;
   if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  k_rhs_tiled<Cfg><<<(unsigned)nblocks, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(map, g, P, fd, sp, coef, dt, tx, ty, tz);
+  k_rhs_tiled<Cfg, STAGE><<<(unsigned)nblocks, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(map, g, P, fd, sp, coef, dt, tx,
+                                                                                     ty, tz, sa);
   return cudaSuccess;
 }
 

@@ -216,8 +216,9 @@ class Z4c:
     def use_graph(self, enable: bool):
         self._check(self.lib.z4c_use_graph(self.h, int(bool(enable))))
 
-    def set_fused(self, enable: bool):
-        self._check(self.lib.z4c_set_fused(self.h, int(bool(enable))))
+    def set_fused(self, mode):
+        """0: K2, K3, K1 separate; 1 (or True): K2 + K3 with ghost push; 2: one kernel per RK stage (default)."""
+        self._check(self.lib.z4c_set_fused(self.h, int(mode)))
 
     def step_timed(self, nsteps: int = 1):
         """z4c_step_timed: returns {"rhs": ms, "update": ms, "ghost": ms} summed over nsteps."""
