@@ -1,0 +1,62 @@
+"""Host-side logic of bench.py without a GPU: the multi-rank aggregation (MAX time, SUM units) on a 2-rank gloo
+group, the workload table, the CPU reference arm."""
+import json
+import os
+import subprocess
+import sys
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    sys.path.insert(0, ROOT)
+    import bench
+    ms, units = bench.aggregate(10.0 + 5.0 * rank, 1000.0 * (rank + 1), dist)
+    q.put((rank, ms, units))
+    dist.destroy_process_group()
+
+
+def test_aggregate_two_ranks_gloo():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, 2, 29731, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in range(2)]
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    for _, ms, units in res:
+        assert ms == 15.0 and units == 3000.0        # max over ranks, sum over ranks (replicas, weak scaling)
+
+
+def test_aggregate_single_rank():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.aggregate(3.0, 7.0, None) == (3.0, 7.0)
+
+
+def test_workload_table_matches_baseline_configs():
+    sys.path.insert(0, ROOT)
+    import bench
+    p, u, label = bench.workload("linear_wave_64")
+    assert p.N == (64, 64, 64) and p.n == 16 and p.nblocks == 64 and "configs[1]" in label
+    p, u, _ = bench.workload("noise_16_2x2x2")
+    assert p.nblocks == 8 and u.shape == (22, 32, 32, 32)
+    ps, us, what = bench.oracle_sample("linear_wave_64")
+    assert ps.N == (64, 16, 16)
+
+
+def test_reference_arm_prints_contract_line():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "1"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["unit"] == "zone-cycles/s" and line["value"] > 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0

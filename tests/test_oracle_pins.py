@@ -412,3 +412,18 @@ def test_flop_census(oracle):
     c = oracle.count_flops(p, _smooth_random_state(p), 3, 4, 5)
     total = sum(c["rhs"].values())
     assert 4000 < total < 9000, c
+
+
+# ---------------------------------------------------------------- flop census used by bench.py's roofline
+def test_flop_census(oracle):
+    """bench.py's RHS_FLOPS_PER_CELL is the oracle's own operation count (add = mul = div = 1, no FMA fusion)."""
+    import bench
+    p = I.params_noise(8, (1, 1, 1))
+    u = I.smooth_random_data(p, 5, 0.1)
+    c = oracle.count_flops(p, I.minkowski(p), 1, 1, 1)["rhs"]        # beta >= 0 on all axes
+    assert c["add"] + c["mul"] + c["div"] == bench.RHS_FLOPS_PER_CELL
+    # the only data dependence: the mirrored upwind stencil (beta^k < 0) spends one more multiplication per
+    # field and axis; the roofline uses the smaller count
+    c2 = oracle.count_flops(p, u, 3, 4, 5)["rhs"]
+    tot2 = c2["add"] + c2["mul"] + c2["div"]
+    assert bench.RHS_FLOPS_PER_CELL <= tot2 <= bench.RHS_FLOPS_PER_CELL + 66 and c2["add"] == c["add"]
