@@ -38,6 +38,7 @@ struct z4c_ctx {
   double* ybuf[2];    // ybuf[0] = y (caller's state), ybuf[1] = second state buffer in the workspace
   CUtensorMap ymap[2];  // TMA descriptors of the two state buffers (tuned K2)
   CUtensorMap ymap2[2]; // same with the 128-thread tile box
+  RegMaps rmap, rmap2;  // TMA descriptors of the RK registers P, Q for the two tile shapes
   int have_ymap;
   std::string err;
 };
@@ -107,7 +108,7 @@ int launch_ghost_fill(z4c_ctx* c) {
 int launch_rhs(z4c_ctx* c, double coef, double dt) {
   const Pack& g = c->g;
   if (c->variant != 1 && c->have_ymap) {
-    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{});
+    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], c->rmap, g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{});
     if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
     return check_launch(c, "k_rhs_tiled");
   }
@@ -142,18 +143,19 @@ int launch_stage_update(z4c_ctx* c, int stage, bool push) {
 // One RK stage as ONE kernel: RHS from ybuf[in] (TMA tiles), recurrence + enforcement in registers, updated
 // state and its ghost images written to ybuf[1-in].
 template <class Cfg>
-cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, int stage, const StageArgs& sa) {
+cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, const RegMaps& rm, int stage,
+                                 const StageArgs& sa) {
   switch (stage) {
-    case 1: return launch_rhs_tiled_t<Cfg, 1>(map, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
-    case 2: return launch_rhs_tiled_t<Cfg, 2>(map, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
-    case 3: return launch_rhs_tiled_t<Cfg, 3>(map, c->g, c->P, c->fd, c->sp, -0.5, c->dt, c->stream, sa);
-    default: return launch_rhs_tiled_t<Cfg, 4>(map, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa);
+    case 1: return launch_rhs_tiled_t<Cfg, 1>(map, rm, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
+    case 2: return launch_rhs_tiled_t<Cfg, 2>(map, rm, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
+    case 3: return launch_rhs_tiled_t<Cfg, 3>(map, rm, c->g, c->P, c->fd, c->sp, -0.5, c->dt, c->stream, sa);
+    default: return launch_rhs_tiled_t<Cfg, 4>(map, rm, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa);
   }
 }
 int launch_fused_stage(z4c_ctx* c, int stage, int in) {
   StageArgs sa{c->Q, c->ybuf[1 - in], c->prm.chi_floor, c->flag};
-  cudaError_t e = c->variant == 2 ? launch_fused_stage_t<RhsTile2>(c, c->ymap2[in], stage, sa)
-                                  : launch_fused_stage_t<RhsTile>(c, c->ymap[in], stage, sa);
+  cudaError_t e = c->variant == 2 ? launch_fused_stage_t<RhsTile2>(c, c->ymap2[in], c->rmap2, stage, sa)
+                                  : launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
   return check_launch(c, "k_rhs_tiled<stage>");
 }
@@ -311,7 +313,11 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->ybuf[0], &c->ymap[0]) &&
                  make_state_tensor_map<RhsTile>(c->g, c->ybuf[1], &c->ymap[1]) &&
                  make_state_tensor_map<RhsTile2>(c->g, c->ybuf[0], &c->ymap2[0]) &&
-                 make_state_tensor_map<RhsTile2>(c->g, c->ybuf[1], &c->ymap2[1]) ? 1 : 0;
+                 make_state_tensor_map<RhsTile2>(c->g, c->ybuf[1], &c->ymap2[1]) &&
+                 make_register_tensor_map<RhsTile>(c->g, c->P, &c->rmap.p) &&
+                 make_register_tensor_map<RhsTile>(c->g, c->Q, &c->rmap.q) &&
+                 make_register_tensor_map<RhsTile2>(c->g, c->P, &c->rmap2.p) &&
+                 make_register_tensor_map<RhsTile2>(c->g, c->Q, &c->rmap2.q) ? 1 : 0;
   cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
   if (e != cudaSuccess) {
     delete c;

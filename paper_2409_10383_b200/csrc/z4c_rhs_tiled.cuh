@@ -58,7 +58,15 @@ struct TileCfg {
   static constexpr int TILE_ELEMS = HX * HY * HZ;
   static constexpr int TILE_BYTES = TILE_ELEMS * 8;
   static constexpr int STAGE_BYTES = (TILE_BYTES + 127) / 128 * 128;
-  static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 128;
+  static constexpr int BAR_OFF = NSTAGE * STAGE_BYTES;            // NSTAGE + 1 mbarriers
+  static constexpr int REG_BYTES = NF * THREADS * 8;              // one RK-register tile [22][TZ][TY][TX]
+  static constexpr int P_OFF = BAR_OFF + 128;                     // P tile, later the staged new state
+  static constexpr int Q_OFF = P_OFF + REG_BYTES;
+  static constexpr int LIST_OFF = Q_OFF + REG_BYTES;              // push lists: 3 axes x {src, blk, idx} x 32 ints
+  static constexpr int MAXLIST = 32;
+  static constexpr int SMEM_BYTES_RHS = BAR_OFF + 128;            // STAGE 0
+  static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
+  static_assert(TX + 2 * NG <= MAXLIST && TY + 2 * NG <= MAXLIST && TZ + 2 * NG <= MAXLIST, "push list size");
 };
 
 // field streaming order: the shift first (its sign and size weight every other field's advection)
@@ -151,11 +159,16 @@ struct StageArgs {
 // expression forms as k_stage_update, applied to the cell while its 22 values are still in registers.
 template <class Cfg, int STAGE>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
-    k_rhs_tiled(const __grid_constant__ CUtensorMap map, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
+    k_rhs_tiled(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap pmap,
+                const __grid_constant__ CUtensorMap qmap, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
                 double c, double dt, int tiles_x, int tiles_y, int tiles_z, StageArgs sa) {
   static_assert(Cfg::NSTAGE >= 3, "the three shift components are staged together");
   extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
-  uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::NSTAGE * Cfg::STAGE_BYTES);
+  uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::BAR_OFF);
+  uint64_t* pqbar = full + Cfg::NSTAGE;
+  double* sP = reinterpret_cast<double*>(tiles + Cfg::P_OFF);
+  double* sQ = reinterpret_cast<double*>(tiles + Cfg::Q_OFF);
+  int* lists = reinterpret_cast<int*>(tiles + Cfg::LIST_OFF);
   const int tid = threadIdx.x;
   const int lx = tid % Cfg::TX, ly = (tid / Cfg::TX) % Cfg::TY, lz = tid / (Cfg::TX * Cfg::TY);
   int t = blockIdx.x;
@@ -168,6 +181,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < Cfg::NSTAGE; ++s) mbar_init(&full[s], 1);
+    mbar_init(pqbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -176,6 +190,32 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     for (int s = 0; s < Cfg::NSTAGE; ++s) {
       mbar_expect_tx(&full[s], Cfg::TILE_BYTES);
       tma_load_5d(tiles + s * Cfg::STAGE_BYTES, &map, &full[s], cx, cy, cz, b, stream_field(s));
+    }
+    // the RK registers of this tile, all 22 fields in one box each: they land long before the epilogue needs them
+    if (STAGE >= 2) {
+      mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
+      tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
+      if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
+    }
+    // push lists (O2): per axis, every (source cell of this tile -> destination block, padded index) pair,
+    // the cell's own position included; the destinations of the tile are the product of the three lists
+    if (STAGE >= 1) {
+      int bxyz[3];
+      block_coords(g, b, bxyz[0], bxyz[1], bxyz[2]);
+      const int c0[3] = {cx, cy, cz}, T[3] = {Cfg::TX, Cfg::TY, Cfg::TZ};
+      for (int a = 0; a < 3; ++a) {
+        int* L = lists + a * 3 * Cfg::MAXLIST;
+        int cnt = 0;
+        for (int l = c0[a]; l < c0[a] + T[a] && l < g.n; ++l) {
+          int tb[4], tl[4];
+          const int nt = push_targets(l, bxyz[a], g.n, g.nb[a], g.bc, tb, tl);
+          for (int q = 0; q < nt; ++q) {
+            L[cnt] = l - c0[a]; L[Cfg::MAXLIST + cnt] = tb[q]; L[2 * Cfg::MAXLIST + cnt] = tl[q];
+            ++cnt;
+          }
+        }
+        lists[9 * Cfg::MAXLIST + a] = cnt;
+      }
     }
   }
   const int toff = (lz + NG) * Cfg::SZ + (ly + NG) * Cfg::SY + lx + NG;
@@ -192,11 +232,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   double u[NF], out[NF];
   Derivs D;
   FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
-  if (!active) return;
-  z4c_sources(sp, u, D, out);
+  if (active) z4c_sources(sp, u, D, out);
   const long long ci = (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
   double* pc = Preg + ci;
   if (STAGE == 0) {
+    if (!active) return;
     if (c != 0.0) {
 #pragma unroll
       for (int f = 0; f < NF; ++f) pc[f * g.is] = c * pc[f * g.is] + dt * out[f];
@@ -206,54 +246,55 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     }
     return;
   }
-  double* qc = sa.Q + ci;
+  if (STAGE >= 2) mbar_wait(pqbar, 0);
+  if (active) {
+    double* qc = sa.Q + ci;
 #pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    if (STAGE == 1) {
-      const double P = dt * out[f];
-      qc[f * g.is] = P;
-      u[f] = u[f] + 0.5 * P;
-    } else if (STAGE == 2) {
-      const double P = dt * out[f];
-      const double Q = qc[f * g.is];
-      pc[f * g.is] = P;
-      u[f] = u[f] + 0.5 * (P - Q);
-      qc[f * g.is] = Q / 6.0;
-    } else if (STAGE == 3) {
-      const double P = -0.5 * pc[f * g.is] + dt * out[f];
-      const double Q = qc[f * g.is];
-      pc[f * g.is] = P;
-      u[f] = u[f] + P;
-      qc[f * g.is] = Q - P;
-    } else {
-      const double P = 2.0 * pc[f * g.is] + dt * out[f];
-      const double Q = qc[f * g.is];
-      u[f] = u[f] + (Q + P / 6.0);
+    for (int f = 0; f < NF; ++f) {
+      if (STAGE == 1) {
+        const double P = dt * out[f];
+        qc[f * g.is] = P;
+        u[f] = u[f] + 0.5 * P;
+      } else if (STAGE == 2) {
+        const double P = dt * out[f];
+        const double Q = sQ[f * Cfg::THREADS + tid];
+        pc[f * g.is] = P;
+        u[f] = u[f] + 0.5 * (P - Q);
+        qc[f * g.is] = Q / 6.0;
+      } else if (STAGE == 3) {
+        const double P = -0.5 * sP[f * Cfg::THREADS + tid] + dt * out[f];
+        const double Q = sQ[f * Cfg::THREADS + tid];
+        pc[f * g.is] = P;
+        u[f] = u[f] + P;
+        qc[f * g.is] = Q - P;
+      } else {
+        const double P = 2.0 * sP[f * Cfg::THREADS + tid] + dt * out[f];
+        const double Q = sQ[f * Cfg::THREADS + tid];
+        u[f] = u[f] + (Q + P / 6.0);
+      }
     }
+    bool bad = enforce_cell(u, sa.chi_floor);
+    bad |= any_nonfinite(u);
+    if (bad) *sa.flag = 1;
+    // stage the new state of the tile (each thread overwrites only its own slots of the P tile)
+#pragma unroll
+    for (int f = 0; f < NF; ++f) sP[f * Cfg::THREADS + tid] = u[f];
   }
-  bool bad = enforce_cell(u, sa.chi_floor);
-  bad |= any_nonfinite(u);
-  if (bad) *sa.flag = 1;
-  double* yo = sa.y_out + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
+  __syncthreads();
+  // cooperative write-out of the tile and all of its ghost images, x fastest: coalesced rows
+  const int* Lx = lists;
+  const int* Ly = lists + 3 * Cfg::MAXLIST;
+  const int* Lz = lists + 6 * Cfg::MAXLIST;
+  const int ncx = lists[9 * Cfg::MAXLIST], ncy = lists[9 * Cfg::MAXLIST + 1], ncz = lists[9 * Cfg::MAXLIST + 2];
+  const int total = ncx * ncy * ncz;
+  for (int q = tid; q < total; q += Cfg::THREADS) {
+    const int qx = q % ncx, r = q / ncx, qy = r % ncy, qz = r / ncy;
+    const int src = (Lz[qz] * Cfg::TY + Ly[qy]) * Cfg::TX + Lx[qx];
+    const long long tb = ((long long)Lz[Cfg::MAXLIST + qz] * g.nb[1] + Ly[Cfg::MAXLIST + qy]) * g.nb[0] + Lx[Cfg::MAXLIST + qx];
+    double* d = sa.y_out + tb * g.m3 +
+                ((long long)Lz[2 * Cfg::MAXLIST + qz] * g.m + Ly[2 * Cfg::MAXLIST + qy]) * g.m + Lx[2 * Cfg::MAXLIST + qx];
 #pragma unroll
-  for (int f = 0; f < NF; ++f) yo[f * g.fs] = u[f];
-  const bool edge = i < NG || i >= g.n - NG || j < NG || j >= g.n - NG || k < NG || k >= g.n - NG;
-  if (edge) {
-    int bx, by, bz;
-    block_coords(g, b, bx, by, bz);
-    int tbx[4], tlx[4], tby[4], tly[4], tbz[4], tlz[4];
-    const int ncx = push_targets(i, bx, g.n, g.nb[0], g.bc, tbx, tlx);
-    const int ncy = push_targets(j, by, g.n, g.nb[1], g.bc, tby, tly);
-    const int ncz = push_targets(k, bz, g.n, g.nb[2], g.bc, tbz, tlz);
-    for (int a = 0; a < ncz; ++a)
-      for (int bb = 0; bb < ncy; ++bb)
-        for (int cc = 0; cc < ncx; ++cc) {
-          if (a + bb + cc == 0) continue;
-          const long long tb = ((long long)tbz[a] * g.nb[1] + tby[bb]) * g.nb[0] + tbx[cc];
-          double* d = sa.y_out + tb * g.m3 + ((long long)tlz[a] * g.m + tly[bb]) * g.m + tlx[cc];
-#pragma unroll
-          for (int f = 0; f < NF; ++f) d[f * g.fs] = u[f];
-        }
+    for (int f = 0; f < NF; ++f) d[f * g.fs] = sP[f * Cfg::THREADS + src];
   }
 }
 
@@ -289,22 +330,47 @@ inline bool make_state_tensor_map(const Pack& g, const double* y, CUtensorMap* o
   return r == CUDA_SUCCESS;
 }
 
+// 5-D tensor map (i, j, k, block, field) of an RK register (interior cells only) with a whole-tile box.
+template <class Cfg>
+inline bool make_register_tensor_map(const Pack& g, const double* reg, CUtensorMap* out) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                               const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                               CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess)
+    return false;
+  const cuuint64_t n = (cuuint64_t)g.n;
+  const cuuint64_t dims[5] = {n, n, n, (cuuint64_t)g.nblk, (cuuint64_t)NF};
+  const cuuint64_t strides[4] = {n * 8, n * n * 8, n * n * n * 8, (cuuint64_t)g.is * 8};
+  const cuuint32_t box[5] = {(cuuint32_t)Cfg::TX, (cuuint32_t)Cfg::TY, (cuuint32_t)Cfg::TZ, 1, (cuuint32_t)NF};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  const CUresult r = ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)reg, dims, strides, box, estr,
+                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+struct RegMaps { CUtensorMap p, q; };
+
 template <class Cfg, int STAGE>
-inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const Pack& g, double* P, const FdConst& fd,
+inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm, const Pack& g, double* P, const FdConst& fd,
                                       const SrcParams& sp, double coef, double dt, cudaStream_t st,
                                       const StageArgs& sa) {
   static bool attr_set = false;
+  constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         Cfg::SMEM_BYTES);
+                                         smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
   const long long nblocks = (long long)tx * ty * tz * g.nblk;
   if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  k_rhs_tiled<Cfg, STAGE><<<(unsigned)nblocks, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(map, g, P, fd, sp, coef, dt, tx,
-                                                                                     ty, tz, sa);
+  k_rhs_tiled<Cfg, STAGE><<<(unsigned)nblocks, Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef, dt, tx,
+                                                                          ty, tz, sa);
   return cudaSuccess;
 }
 
