@@ -37,7 +37,7 @@ struct z4c_ctx {
   int graph_launches;
   double* ybuf[2];    // ybuf[0] = y (caller's state), ybuf[1] = second state buffer in the workspace
   CUtensorMap ymap[2];  // TMA descriptors of the two state buffers (tuned K2)
-  CUtensorMap ymap2[2]; // same with the 128-thread tile box
+  CUtensorMap ymap2[2]; // same with the 16x4x4 tile box (variant 2)
   RegMaps rmap, rmap2;  // TMA descriptors of the RK registers P, Q for the two tile shapes
   int have_ymap;
   std::string err;

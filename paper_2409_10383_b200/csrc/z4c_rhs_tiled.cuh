@@ -299,11 +299,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 }
 
 // ---- host side -------------------------------------------------------------------------------------
-// 256 threads, 255 registers, 1 CTA/SM. (Measured on 64^3: 128-thread tiles capped at 168 / 128 registers for
-// 3 / 4 CTAs per SM were slower, 0.183 / 0.219 ms against 0.170 ms per launch: the spills cost more than the
-// extra warps hide.)
-using RhsTile = TileCfg<16, 4, 4, 3>;
-using RhsTile2 = TileCfg<16, 4, 2, 3, 2>;   // 128 threads, 2 CTAs/SM: one CTA's epilogue overlaps the other's stencils
+// Default: 16x4x2 tile, 128 threads at 255 registers, 2 CTAs per SM, so one CTA's prologue (first TMA wait) and
+// epilogue (write-out) overlap the other's stencil work. Measured (bench.py, one kernel per stage, B200):
+//   64^3 wave: 0.202 ms per launch against 0.213 ms for the 16x4x4 tile (256 threads, 1 CTA per SM);
+//   256^3 two punctures: 9.94 against 10.76 ms.  128-thread tiles capped at 168 / 128 registers (3 / 4 CTAs per
+//   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
+using RhsTile = TileCfg<16, 4, 2, 3, 2>;
+using RhsTile2 = TileCfg<16, 4, 4, 3, 1>;
 
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 
