@@ -85,6 +85,36 @@ __global__ void __launch_bounds__(256) k_ghost_fill(Pack g, double* __restrict__
 // yc points at the cell in field 0. Produces the centre values, the centred derivatives, and
 // out[f] = c_adv(f) * beta^k D^{+-}_k u_f + Q_KO u_f.
 // ---------------------------------------------------------------------------------------------
+template <bool ALL_D1, int F>
+__device__ __forceinline__ void gather_fields(const double* __restrict__ yc, const long long fs, const int* st,
+                                              const FdConst& fd, const SrcParams& P, const double* ab,
+                                              const bool* pos, const double* u, Derivs& D, double* out) {
+  if constexpr (F < NF) {
+    const double* p = yc + F * fs;
+    double adv = 0.0, ko = 0.0, d2[6];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      AxisRaw r;
+      if (need_d2(F)) r = axis_raw<true, true>(p, st[a], u[F], pos[a]);
+      else if (need_d1(F) || ALL_D1) r = axis_raw<true, false>(p, st[a], u[F], pos[a]);
+      else r = axis_raw<false, false>(p, st[a], u[F], pos[a]);
+      if (need_d1(F) || ALL_D1) D.d1[F][a] = r.d1 * fd.inv12h;
+      if (need_d2(F)) d2[sym(a, a)] = r.d2 * fd.inv12h2;
+      adv += ab[a] * r.up;
+      ko += r.ko;
+    }
+    const double cadv = (F == ALPHA) ? P.lapse_advect : (F >= BETAX ? P.shift_advect : 1.0);
+    out[F] = cadv * (adv * fd.inv12h) + ko * fd.ko;
+    if (need_d2(F)) {
+      d2[sym(0, 1)] = mixed_raw(p, st[0], st[1]) * fd.inv144h2;
+      d2[sym(0, 2)] = mixed_raw(p, st[0], st[2]) * fd.inv144h2;
+      d2[sym(1, 2)] = mixed_raw(p, st[1], st[2]) * fd.inv144h2;
+      consume_d2<F>(d2, D);
+    }
+    gather_fields<ALL_D1, F + 1>(yc, fs, st, fd, P, ab, pos, u, D, out);
+  }
+}
+
 template <bool ALL_D1>
 __device__ __forceinline__ void gather_global(const double* __restrict__ yc, const long long fs, const int sy,
                                               const int sz, const FdConst& fd, const SrcParams& P, double* u,
@@ -99,29 +129,8 @@ __device__ __forceinline__ void gather_global(const double* __restrict__ yc, con
     pos[a] = u[BETAX + a] >= 0.0;
   }
   const int st[3] = {1, sy, sz};
-#pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    const double* p = yc + f * fs;
-    double adv = 0.0, ko = 0.0;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      AxisRaw r;
-      if (need_d2(f)) r = axis_raw<true, true>(p, st[a], u[f], pos[a]);
-      else if (need_d1(f) || ALL_D1) r = axis_raw<true, false>(p, st[a], u[f], pos[a]);
-      else r = axis_raw<false, false>(p, st[a], u[f], pos[a]);
-      if (need_d1(f) || ALL_D1) D.d1[f][a] = r.d1 * fd.inv12h;
-      if (need_d2(f)) D.d2[f][sym(a, a)] = r.d2 * fd.inv12h2;
-      adv += ab[a] * r.up;
-      ko += r.ko;
-    }
-    const double cadv = (f == ALPHA) ? P.lapse_advect : (f >= BETAX ? P.shift_advect : 1.0);
-    out[f] = cadv * (adv * fd.inv12h) + ko * fd.ko;
-    if (need_d2(f)) {
-      D.d2[f][sym(0, 1)] = mixed_raw(p, 1, sy) * fd.inv144h2;
-      D.d2[f][sym(0, 2)] = mixed_raw(p, 1, sz) * fd.inv144h2;
-      D.d2[f][sym(1, 2)] = mixed_raw(p, sy, sz) * fd.inv144h2;
-    }
-  }
+  derivs_begin(u + GXX, D);
+  gather_fields<ALL_D1, 0>(yc, fs, st, fd, P, ab, pos, u, D, out);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -108,7 +108,7 @@ int launch_ghost_fill(z4c_ctx* c) {
 int launch_rhs(z4c_ctx* c, double coef, double dt) {
   const Pack& g = c->g;
   if (c->variant != 1 && c->have_ymap) {
-    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], c->rmap, g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{});
+    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], c->rmap, g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{c->y, nullptr, nullptr, 0.0, nullptr});
     if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
     return check_launch(c, "k_rhs_tiled");
   }
@@ -153,7 +153,7 @@ cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, const RegMa
   }
 }
 int launch_fused_stage(z4c_ctx* c, int stage, int in) {
-  StageArgs sa{c->Q, c->ybuf[1 - in], c->prm.chi_floor, c->flag};
+  StageArgs sa{c->ybuf[in], c->Q, c->ybuf[1 - in], c->prm.chi_floor, c->flag};
   cudaError_t e = c->variant == 2 ? launch_fused_stage_t<RhsTile2>(c, c->ymap2[in], c->rmap2, stage, sa)
                                   : launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");

@@ -17,12 +17,43 @@ struct SrcParams {
 __host__ __device__ constexpr bool need_d1(int f) { return !(f >= AXX && f <= AZZ); }
 __host__ __device__ constexpr bool need_d2(int f) { return f <= GZZ || f >= ALPHA; }
 
-// Derivative bundle of one cell (S2 -> S3). Entries of fields that need no such derivative are
-// never read, so after unrolling they do not occupy registers.
+// Derivative bundle of one cell (S2 -> S3). Second derivatives are contracted with gt^{ij} as soon as a field's
+// stencils are done (the inverse metric needs only centre values), so only those of chi and alpha are kept:
+// 66 -> 24 live doubles. Entries of fields that need no such derivative are never read, so after unrolling
+// they do not occupy registers.
 struct Derivs {
+  double gi[6];      // gt^{ij}, filled before the first field is differentiated
   double d1[NF][3];  // centred d_k u_f
-  double d2[NF][6];  // centred d_k d_l u_f, packed (xx,xy,xz,yy,yz,zz)
+  double d2chi[6];   // centred d_k d_l chi, packed (xx,xy,xz,yy,yz,zz)
+  double d2alpha[6]; // centred d_k d_l alpha
+  double lapg[6];    // gt^{lm} d_l d_m gt_p
+  double lapb[3];    // gt^{jk} d_j d_k beta^i
+  double ddivb[3];   // d_j d_k beta^k   (must be zeroed before the shift is differentiated)
 };
+
+__device__ __forceinline__ void derivs_begin(const double* g, Derivs& D) {
+  inv3(g, D.gi);
+  D.ddivb[0] = D.ddivb[1] = D.ddivb[2] = 0.0;
+}
+
+// Hand the six second derivatives of field F to the bundle.
+template <int F>
+__device__ __forceinline__ void consume_d2(const double* d2, Derivs& D) {
+  if (F == CHI) {
+#pragma unroll
+    for (int p = 0; p < 6; ++p) D.d2chi[p] = d2[p];
+  } else if (F == ALPHA) {
+#pragma unroll
+    for (int p = 0; p < 6; ++p) D.d2alpha[p] = d2[p];
+  } else if (F >= GXX && F <= GZZ) {
+    D.lapg[F - GXX] = contract(D.gi, d2);
+  } else if (F >= BETAX) {
+    constexpr int i = F - BETAX;
+    D.lapb[i] = contract(D.gi, d2);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) D.ddivb[j] += d2[sym(j, i)];
+  }
+}
 
 // Geometry shared by the RHS and the constraints.
 struct Geom {
@@ -40,7 +71,8 @@ struct Geom {
 __device__ __forceinline__ void geometry(const double* u, const Derivs& D, Geom& G) {
   const double* g = u + GXX;
   const double* A = u + AXX;
-  inv3(g, G.gi);
+#pragma unroll
+  for (int p = 0; p < 6; ++p) G.gi[p] = D.gi[p];
   double dg[6][3];
 #pragma unroll
   for (int p = 0; p < 6; ++p)
@@ -48,17 +80,14 @@ __device__ __forceinline__ void geometry(const double* u, const Derivs& D, Geom&
     for (int k = 0; k < 3; ++k) dg[p][k] = D.d1[GXX + p][k];
   double Gl[3][6];
   christoffel(dg, G.gi, Gl, G.Gu, G.Gd);
-  double lapg[6];
-#pragma unroll
-  for (int p = 0; p < 6; ++p) lapg[p] = contract(G.gi, D.d2[GXX + p]);
   double dGam[3][3];
 #pragma unroll
   for (int k = 0; k < 3; ++k)
 #pragma unroll
     for (int j = 0; j < 3; ++j) dGam[k][j] = D.d1[GAMX + k][j];
   double Rt[6], Rchi[6];
-  ricci_conformal(g, G.gi, lapg, dGam, Gl, G.Gu, G.Gd, Rt);
-  ricci_chi(u[CHI], D.d1[CHI], D.d2[CHI], g, G.gi, G.Gu, Rchi);
+  ricci_conformal(g, G.gi, D.lapg, dGam, Gl, G.Gu, G.Gd, Rt);
+  ricci_chi(u[CHI], D.d1[CHI], D.d2chi, g, G.gi, G.Gu, Rchi);
 #pragma unroll
   for (int p = 0; p < 6; ++p) G.Ric[p] = Rt[p] + Rchi[p];
   G.Rscal = u[CHI] * contract(G.gi, G.Ric);
@@ -79,9 +108,36 @@ __device__ __forceinline__ void geometry(const double* u, const Derivs& D, Geom&
 
 // O5: out[f] += F_f(y).  `out` must already hold the upwinded advection and Kreiss-Oliger terms
 // (with the gauge advection switches applied), which the derivative gather produces.
+__device__ __forceinline__ void z4c_sources_post(const SrcParams& P, const double* u, const Derivs& D, const Geom& G,
+                                                 double* out);
 __device__ __forceinline__ void z4c_sources(const SrcParams& P, const double* u, const Derivs& D, double* out) {
   Geom G;
   geometry(u, D, G);
+  z4c_sources_post(P, u, D, G, out);
+}
+
+// The derivatives that only the assembly after geometry() reads: 30 doubles. A kernel may park them in shared
+// memory across geometry(), where the Christoffel / Ricci temporaries peak (STORE = true before, false after).
+constexpr int NPARK = 30;
+template <bool STORE>
+__device__ __forceinline__ void park_late_derivs(Derivs& D, double* slot, const int stride) {
+  int q = 0;
+  auto io = [&](double& x) {
+    if (STORE) slot[q * stride] = x; else x = slot[q * stride];
+    ++q;
+  };
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    io(D.d1[BETAX][a]); io(D.d1[BETAY][a]); io(D.d1[BETAZ][a]);
+    io(D.d1[KHAT][a]); io(D.d1[THETA][a]); io(D.d1[ALPHA][a]);
+    io(D.lapb[a]); io(D.ddivb[a]);
+  }
+#pragma unroll
+  for (int p = 0; p < 6; ++p) io(D.d2alpha[p]);
+}
+
+__device__ __forceinline__ void z4c_sources_post(const SrcParams& P, const double* u, const Derivs& D, const Geom& G,
+                                                 double* out) {
   const double* g = u + GXX;
   const double* A = u + AXX;
   const double chi = u[CHI], alpha = u[ALPHA], Theta = u[THETA], K = G.K;
@@ -104,7 +160,7 @@ __device__ __forceinline__ void z4c_sources(const SrcParams& P, const double* u,
     const double dadchi = 0.5 * contract(gi, dd);
 #pragma unroll
     for (int p = 0; p < 6; ++p)
-      DDa[p] = D.d2[ALPHA][p] - (G.Gu[0][p] * da[0] + G.Gu[1][p] * da[1] + G.Gu[2][p] * da[2]) +
+      DDa[p] = D.d2alpha[p] - (G.Gu[0][p] * da[0] + G.Gu[1][p] * da[1] + G.Gu[2][p] * da[2]) +
                0.5 * ichi * (dd[p] - g[p] * dadchi);
   }
 
@@ -144,11 +200,7 @@ __device__ __forceinline__ void z4c_sources(const SrcParams& P, const double* u,
   }
 
   {
-    // d_j (d_k beta^k)
-    double ddivb[3];
-#pragma unroll
-    for (int j = 0; j < 3; ++j)
-      ddivb[j] = D.d2[BETAX][sym(j, 0)] + D.d2[BETAY][sym(j, 1)] + D.d2[BETAZ][sym(j, 2)];
+    const double* ddivb = D.ddivb;   // d_j (d_k beta^k)
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
       double s = 0.0, b = 0.0;
@@ -162,7 +214,7 @@ __device__ __forceinline__ void z4c_sources(const SrcParams& P, const double* u,
       }
       b += contract(G.Gu[i], G.Aup);
       s += 2.0 * alpha * b;
-      s += contract(gi, D.d2[BETAX + i]);
+      s += D.lapb[i];
       s += (2.0 / 3.0) * G.Gd[i] * divb;
       s -= 2.0 * P.kappa1 * alpha * (u[GAMX + i] - G.Gd[i]);
       out[GAMX + i] += s;

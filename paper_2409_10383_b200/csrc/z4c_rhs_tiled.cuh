@@ -62,9 +62,10 @@ struct TileCfg {
   static constexpr int REG_BYTES = NF * THREADS * 8;              // one RK-register tile [22][TZ][TY][TX]
   static constexpr int P_OFF = BAR_OFF + 128;                     // P tile, later the staged new state
   static constexpr int Q_OFF = P_OFF + REG_BYTES;
-  static constexpr int LIST_OFF = Q_OFF + REG_BYTES;              // push lists: 3 axes x {src, blk, idx} x 32 ints
+  static constexpr int S_OFF = Q_OFF + REG_BYTES;                 // per-thread parking of the advection + KO sums
+  static constexpr int LIST_OFF = S_OFF + REG_BYTES;              // push lists: 3 axes x {src, blk, idx} x 32 ints
   static constexpr int MAXLIST = 32;
-  static constexpr int SMEM_BYTES_RHS = BAR_OFF + 128;            // STAGE 0
+  static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
   static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
   static_assert(TX + 2 * NG <= MAXLIST && TY + 2 * NG <= MAXLIST && TZ + 2 * NG <= MAXLIST, "push list size");
 };
@@ -107,13 +108,16 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
   axis_tile<Cfg::SZ, W1, W2>(t, c, bw[2], aw[2], fd, d1z, d2z, adv, ko);
   if (W1) { D.d1[F][0] = d1x; D.d1[F][1] = d1y; D.d1[F][2] = d1z; }
   if (W2) {
-    D.d2[F][sym(0, 0)] = d2x; D.d2[F][sym(1, 1)] = d2y; D.d2[F][sym(2, 2)] = d2z;
-    D.d2[F][sym(0, 1)] = mixed_tile<1, Cfg::SY>(t) * fd.inv144h2;
-    D.d2[F][sym(0, 2)] = mixed_tile<1, Cfg::SZ>(t) * fd.inv144h2;
-    D.d2[F][sym(1, 2)] = mixed_tile<Cfg::SY, Cfg::SZ>(t) * fd.inv144h2;
+    double d2[6];
+    d2[sym(0, 0)] = d2x; d2[sym(1, 1)] = d2y; d2[sym(2, 2)] = d2z;
+    d2[sym(0, 1)] = mixed_tile<1, Cfg::SY>(t) * fd.inv144h2;
+    d2[sym(0, 2)] = mixed_tile<1, Cfg::SZ>(t) * fd.inv144h2;
+    d2[sym(1, 2)] = mixed_tile<Cfg::SY, Cfg::SZ>(t) * fd.inv144h2;
+    consume_d2<F>(d2, D);
   }
   const double cadv = (F == ALPHA) ? sp.lapse_advect : (F >= BETAX ? sp.shift_advect : 1.0);
-  out[F] = cadv * adv + ko * fd.ko;
+  // parked in shared memory until the sources are assembled: 22 doubles fewer live through the tensor algebra
+  out[F * Cfg::THREADS] = cadv * adv + ko * fd.ko;
 }
 
 template <class Cfg, int IT>
@@ -148,6 +152,7 @@ struct FieldLoop<Cfg, NF> {
 // reads y_in through the tensor map and writes the updated, enforced state and its ghost images to y_out, so
 // no CTA ever reads a cell another CTA is writing), the chi floor and the error flag.
 struct StageArgs {
+  const double* y_in;   // the state buffer the tensor map describes (centre values of gt_ij are read up front)
   double* Q;
   double* y_out;
   double chi_floor;
@@ -229,10 +234,42 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     bw[a] = beta * (0.5 * fd.inv12h);
     aw[a] = fabs(beta) * (0.5 * fd.inv12h);
   }
-  double u[NF], out[NF];
+  double u[NF];
+  double* park = reinterpret_cast<double*>(tiles + Cfg::S_OFF) + tid;
   Derivs D;
-  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
-  if (active) z4c_sources(sp, u, D, out);
+  {
+    // gt^{ij} is needed while the very first fields stream in: fetch the six centre values directly
+    const double* yc = sa.y_in + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
+    double gc[6];
+#pragma unroll
+    for (int p = 0; p < 6; ++p) gc[p] = active ? __ldg(yc + (GXX + p) * g.fs) : (p == 0 || p == 3 || p == 5 ? 1.0 : 0.0);
+    derivs_begin(gc, D);
+  }
+  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park);
+  double out[NF];
+  constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
+  if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring
+  if (active) {
+#pragma unroll
+    for (int f = 0; f < NF; ++f) out[f] = 0.0;
+    Geom G;
+    if (PARK) {
+      // the tile ring is idle now: park what only the final assembly reads while geometry() peaks
+      // (this thread's last stencil loads are complete -- their values were consumed above -- and no TMA is
+      // pending; other threads' reads of the ring are fenced by the barrier above)
+      double* slot = reinterpret_cast<double*>(tiles) + tid;
+      park_late_derivs<true>(D, slot, Cfg::THREADS);
+      asm volatile("" ::: "memory");
+      geometry(u, D, G);
+      asm volatile("" ::: "memory");
+      park_late_derivs<false>(D, slot, Cfg::THREADS);
+    } else {
+      geometry(u, D, G);
+    }
+    z4c_sources_post(sp, u, D, G, out);
+#pragma unroll
+    for (int f = 0; f < NF; ++f) out[f] += park[f * Cfg::THREADS];
+  }
   const long long ci = (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
   double* pc = Preg + ci;
   if (STAGE == 0) {
