@@ -407,13 +407,6 @@ def test_constraints_norm_definitions(oracle):
     assert np.isclose(out[3], np.sqrt((pc[1:] ** 2).sum(0)).max(), rtol=5e-3)
 
 
-def test_flop_census(oracle):
-    p = I.params_noise(8, (1, 1, 1))
-    c = oracle.count_flops(p, _smooth_random_state(p), 3, 4, 5)
-    total = sum(c["rhs"].values())
-    assert 4000 < total < 9000, c
-
-
 # ---------------------------------------------------------------- flop census used by bench.py's roofline
 def test_flop_census(oracle):
     """bench.py's RHS_FLOPS_PER_CELL is the oracle's own operation count (add = mul = div = 1, no FMA fusion)."""
