@@ -3,8 +3,8 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
 
-A "step" is one classical RK4 step (4 x [K2 RHS -> K3 stage update + enforcement + ghost push]) over the whole
-pack. Default workload: BASELINE.json configs[1], the linear gravitational wave on 64^3 cells in 64 blocks of
+A "step" is one classical RK4 step (4 stages of RHS -> stage update + enforcement -> ghost fill; by default one
+fused kernel per stage) over the whole pack. Default workload: BASELINE.json configs[1], the linear gravitational wave on 64^3 cells in 64 blocks of
 16^3 (+3 ghosts). One JSON line is printed by rank 0. See DESIGN.md "Measurement" for every figure's definition.
 """
 from __future__ import annotations
@@ -61,6 +61,15 @@ def workload(name: str):
         tile = tuple(2 if b % 2 == 0 else 1 for b in nb)
         return p, I.tiled_noise_data(p, tile, 1000), f"configs[4]: noise, {nb} blocks of {n}^3, periodic"
     raise SystemExit(f"unknown workload {name}")
+
+
+def profiled_traffic(name: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            return float(json.load(f)[name]["mean_bytes_per_launch"])
+    except Exception:
+        return None
 
 
 def measured_peaks():
@@ -303,8 +312,9 @@ def run_ours(args):
                     "d2h_bytes_per_step": nbytes, "steps": Ke,
                     "what": "z4c_set_initial_data(host) + z4c_step(1) + z4c_get_interior(host) per step, pinned"},
             "gpu_launches": int(launches),
-            "roofline": {"kernel": "K2 z4c_rhs", "bound": "alu", "achieved": rhs_tflops, "peak": fp64_peak,
-                         "unit": "TFLOP/s", "frac": rhs_tflops / fp64_peak, "traffic": None,
+            "roofline": {"kernel": "k_rhs_tiled<STAGE> (one kernel per RK stage)" if args.fuse == 2 and args.variant != 1 else "K2 z4c_rhs", "bound": "alu", "achieved": rhs_tflops, "peak": fp64_peak,
+                         "unit": "TFLOP/s", "frac": rhs_tflops / fp64_peak,
+                         "traffic": profiled_traffic(args.workload),
                          "peak_source": "measured live: z4c_probe_fp64 DFMA loop (nominal %.1f at 1965 MHz)" % FP64_NOMINAL_TFLOPS,
                          "flops_per_cell": RHS_FLOPS_PER_CELL, "ms_per_launch": rhs_ms,
                          "hbm_gbs_algorithmic": rhs_gbs, "share_of_step": kt["rhs"] / total_kt},
