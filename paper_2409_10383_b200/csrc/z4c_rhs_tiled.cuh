@@ -403,6 +403,9 @@ inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm,
     cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          smem);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
