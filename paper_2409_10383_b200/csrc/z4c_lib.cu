@@ -168,6 +168,11 @@ int launch_fused_stage(z4c_ctx* c, int stage, int in) {
     if (e != cudaSuccess) return check_cuda(c, e, "k_stage_persistent launch");
     return check_launch(c, "k_stage_persistent");
   }
+  if (c->variant == 4) {
+    cudaError_t e4 = launch_fused_stage_t<RhsTile5>(c, c->ymap[in], c->rmap, stage, sa);
+    if (e4 != cudaSuccess) return check_cuda(c, e4, "k_rhs_tiled launch");
+    return check_launch(c, "k_rhs_tiled<stage>");
+  }
   cudaError_t e = c->variant == 2 ? launch_fused_stage_t<RhsTile2>(c, c->ymap2[in], c->rmap2, stage, sa)
                                   : launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);   // variant 0
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
@@ -510,7 +515,7 @@ int z4c_sync(z4c_ctx* c) {
 int64_t z4c_launch_count(const z4c_ctx* c) { return c ? c->launches : 0; }
 
 int z4c_set_variant(z4c_ctx* c, int variant) {
-  if (!c || variant < 0 || variant > 3) return Z4C_EINVAL;
+  if (!c || variant < 0 || variant > 4) return Z4C_EINVAL;
   if (variant != c->variant) drop_graph(c);
   c->variant = variant;
   return Z4C_OK;

@@ -49,9 +49,13 @@ __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* m
 }
 
 // ---- tile geometry ---------------------------------------------------------------------------------
-template <int TX_, int TY_, int TZ_, int NSTAGE_, int MINB_ = 1>
+// PQ_TMA_: true = the CTA's P/Q register tiles are TMA-prefetched into shared memory at kernel start;
+// false = they are read in the epilogue as one batch of independent global loads (lines requested into L2 by a
+// prefetch at kernel start), which frees 2 x 22 x THREADS x 8 bytes of shared memory for a deeper tile ring.
+template <int TX_, int TY_, int TZ_, int NSTAGE_, int MINB_ = 1, bool PQ_TMA_ = true>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NSTAGE = NSTAGE_, MINB = MINB_;
+  static constexpr bool PQ_TMA = PQ_TMA_;
   static constexpr int THREADS = TX * TY * TZ;
   static constexpr int HX = TX + 2 * NG, HY = TY + 2 * NG, HZ = TZ + 2 * NG;
   static constexpr int SY = HX, SZ = HX * HY;          // element strides inside the halo tile
@@ -61,8 +65,9 @@ struct TileCfg {
   static constexpr int BAR_OFF = NSTAGE * STAGE_BYTES;            // NSTAGE + 1 mbarriers
   static constexpr int REG_BYTES = NF * THREADS * 8;              // one RK-register tile [22][TZ][TY][TX]
   static constexpr int P_OFF = BAR_OFF + 128;                     // P tile, later the staged new state
-  static constexpr int Q_OFF = P_OFF + REG_BYTES;
-  static constexpr int S_OFF = Q_OFF + REG_BYTES;                 // per-thread parking of the advection + KO sums
+  static constexpr int Q_OFF = P_OFF + (PQ_TMA ? REG_BYTES : 0);
+  // per-thread parking of the advection + KO sums (without PQ_TMA it coincides with the staging tile at P_OFF)
+  static constexpr int S_OFF = Q_OFF + (PQ_TMA ? REG_BYTES : 0);
   static constexpr int LIST_OFF = S_OFF + REG_BYTES;              // push lists: 3 axes x {src, blk, idx} x 32 ints
   static constexpr int MAXLIST = 32;
   static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
@@ -171,8 +176,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
   uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::BAR_OFF);
   uint64_t* pqbar = full + Cfg::NSTAGE;
+  // sP: staging tile of the new state (and the TMA'd P tile with PQ_TMA); sP2 / sQ: where the epilogue reads the old
+  // P and Q -- with PQ_TMA the TMA tiles, otherwise two 22 x THREADS areas of the idle tile ring
   double* sP = reinterpret_cast<double*>(tiles + Cfg::P_OFF);
-  double* sQ = reinterpret_cast<double*>(tiles + Cfg::Q_OFF);
+  double* sP2 = Cfg::PQ_TMA ? sP : reinterpret_cast<double*>(tiles);   // (per-thread slots; the parking is over by then)
+  double* sQ = Cfg::PQ_TMA ? reinterpret_cast<double*>(tiles + Cfg::Q_OFF)
+                           : reinterpret_cast<double*>(tiles) + NF * Cfg::THREADS;
+  static_assert(Cfg::PQ_TMA || Cfg::NSTAGE * Cfg::STAGE_BYTES >= 2 * NF * Cfg::THREADS * 8, "ring too small");
   int* lists = reinterpret_cast<int*>(tiles + Cfg::LIST_OFF);
   const int tid = threadIdx.x;
   const int lx = tid % Cfg::TX, ly = (tid / Cfg::TX) % Cfg::TY, lz = tid / (Cfg::TX * Cfg::TY);
@@ -197,7 +207,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
       tma_load_5d(tiles + s * Cfg::STAGE_BYTES, &map, &full[s], cx, cy, cz, b, stream_field(s));
     }
     // the RK registers of this tile, all 22 fields in one box each: they land long before the epilogue needs them
-    if (STAGE >= 2) {
+    if (STAGE >= 2 && Cfg::PQ_TMA) {
       mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
       tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
       if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
@@ -226,6 +236,15 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   const int toff = (lz + NG) * Cfg::SZ + (ly + NG) * Cfg::SY + lx + NG;
   const int i = cx + lx, j = cy + ly, k = cz + lz;
   const bool active = i < g.n && j < g.n && k < g.n;
+  if (STAGE >= 2 && !Cfg::PQ_TMA && active && lx == 0) {
+    // ask L2 for this tile's rows of the RK registers (one 128-byte line per row and field)
+    const long long c0 = (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(sa.Q + c0 + f * g.is));
+      if (STAGE >= 3) asm volatile("prefetch.global.L2 [%0];" ::"l"(Preg + c0 + f * g.is));
+    }
+  }
   double bw[3], aw[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
@@ -283,9 +302,24 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     }
     return;
   }
-  if (STAGE >= 2) mbar_wait(pqbar, 0);
+  if (STAGE >= 2 && Cfg::PQ_TMA) mbar_wait(pqbar, 0);
   if (active) {
     double* qc = sa.Q + ci;
+    if (!Cfg::PQ_TMA) {
+      // all loads of the RK registers first, as one batch of independent requests, parked in the (now idle) tile
+      // ring at the slots the code below reads (the stores to P/Q may alias the loads as far as the compiler knows)
+      double Pold[NF], Qold[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        Qold[f] = STAGE >= 2 ? __ldcg(qc + f * g.is) : 0.0;
+        Pold[f] = STAGE >= 3 ? __ldcg(pc + f * g.is) : 0.0;
+      }
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        sQ[f * Cfg::THREADS + tid] = Qold[f];
+        if (STAGE >= 3) sP2[f * Cfg::THREADS + tid] = Pold[f];
+      }
+    }
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       if (STAGE == 1) {
@@ -299,13 +333,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
         u[f] = u[f] + 0.5 * (P - Q);
         qc[f * g.is] = Q / 6.0;
       } else if (STAGE == 3) {
-        const double P = -0.5 * sP[f * Cfg::THREADS + tid] + dt * out[f];
+        const double P = -0.5 * sP2[f * Cfg::THREADS + tid] + dt * out[f];
         const double Q = sQ[f * Cfg::THREADS + tid];
         pc[f * g.is] = P;
         u[f] = u[f] + P;
         qc[f * g.is] = Q - P;
       } else {
-        const double P = 2.0 * sP[f * Cfg::THREADS + tid] + dt * out[f];
+        const double P = 2.0 * sP2[f * Cfg::THREADS + tid] + dt * out[f];
         const double Q = sQ[f * Cfg::THREADS + tid];
         u[f] = u[f] + (Q + P / 6.0);
       }
@@ -343,6 +377,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
 using RhsTile2 = TileCfg<16, 4, 4, 3, 1>;
+using RhsTile5 = TileCfg<16, 4, 2, 5, 2, false>;   // 5-deep ring, P/Q by batched global loads (variant 4)
 
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 
