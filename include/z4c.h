@@ -138,7 +138,8 @@ int64_t z4c_launch_count(const z4c_ctx* ctx);
 /* Select the RHS kernel variant: 0 = tuned kernel, TMA-staged 16x4x2 tiles, 128 threads, 2 CTAs per SM
  * (default); 1 = plain global-memory kernel; 2 = tuned kernel with 16x4x4 tiles, 256 threads, 1 CTA per SM;
  * 3 = persistent one-kernel-per-stage variant (CTAs walk a stream of tiles and prefetch the next tile's halo
- * tiles; experimental, measured slower than variant 0).
+ * tiles; experimental, measured slower than variant 0); 4 = variant 0 with the P/Q tiles read by batched global loads
+ * instead of TMA and the late-use derivatives parked in shared memory as they are produced (measured 3 % slower).
  * For A/B measurements; all variants compute the same values. */
 int z4c_set_variant(z4c_ctx* ctx, int variant);
 /* Enable (1) / disable (0) CUDA-graph replay of the RK4 step inside z4c_step. Default 0. */

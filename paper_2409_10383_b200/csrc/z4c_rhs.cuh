@@ -136,6 +136,26 @@ __device__ __forceinline__ void park_late_derivs(Derivs& D, double* slot, const 
   for (int p = 0; p < 6; ++p) io(D.d2alpha[p]);
 }
 
+// The same slots, written as soon as field F's stencils are done (a kernel with a dedicated parking area can keep
+// these values out of registers through the whole field stream, not only through geometry()).
+template <int F>
+__device__ __forceinline__ void park_field_early(const Derivs& D, double* slot, const int stride) {
+  constexpr int col = F == BETAX ? 0 : F == BETAY ? 1 : F == BETAZ ? 2 : F == KHAT ? 3 : F == THETA ? 4 : F == ALPHA ? 5 : -1;
+  if (col >= 0) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) slot[(a * 8 + col) * stride] = D.d1[F][a];
+  }
+  if (F >= BETAX) slot[((F - BETAX) * 8 + 6) * stride] = D.lapb[F - BETAX];
+  if (F == BETAZ) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) slot[(a * 8 + 7) * stride] = D.ddivb[a];
+  }
+  if (F == ALPHA) {
+#pragma unroll
+    for (int p = 0; p < 6; ++p) slot[(24 + p) * stride] = D.d2alpha[p];
+  }
+}
+
 __device__ __forceinline__ void z4c_sources_post(const SrcParams& P, const double* u, const Derivs& D, const Geom& G,
                                                  double* out) {
   const double* g = u + GXX;

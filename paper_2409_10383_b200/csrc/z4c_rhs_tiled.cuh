@@ -68,7 +68,11 @@ struct TileCfg {
   static constexpr int Q_OFF = P_OFF + (PQ_TMA ? REG_BYTES : 0);
   // per-thread parking of the advection + KO sums (without PQ_TMA it coincides with the staging tile at P_OFF)
   static constexpr int S_OFF = Q_OFF + (PQ_TMA ? REG_BYTES : 0);
-  static constexpr int LIST_OFF = S_OFF + REG_BYTES;              // push lists: 3 axes x {src, blk, idx} x 32 ints
+  // without PQ_TMA the freed space holds a dedicated parking area for the late-use derivatives (written as each
+  // field is done, so they stay out of registers through the whole field stream)
+  static constexpr bool EARLY_PARK = !PQ_TMA;
+  static constexpr int E_OFF = S_OFF + REG_BYTES;
+  static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0);   // push lists
   static constexpr int MAXLIST = 32;
   static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
   static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
@@ -123,6 +127,7 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
   const double cadv = (F == ALPHA) ? sp.lapse_advect : (F >= BETAX ? sp.shift_advect : 1.0);
   // parked in shared memory until the sources are assembled: 22 doubles fewer live through the tensor algebra
   out[F * Cfg::THREADS] = cadv * adv + ko * fd.ko;
+  if (Cfg::EARLY_PARK) park_field_early<F>(D, out + (Cfg::E_OFF - Cfg::S_OFF) / 8, Cfg::THREADS);
 }
 
 template <class Cfg, int IT>
@@ -176,13 +181,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
   uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::BAR_OFF);
   uint64_t* pqbar = full + Cfg::NSTAGE;
-  // sP: staging tile of the new state (and the TMA'd P tile with PQ_TMA); sP2 / sQ: where the epilogue reads the old
-  // P and Q -- with PQ_TMA the TMA tiles, otherwise two 22 x THREADS areas of the idle tile ring
+  // sP: staging tile of the new state (with PQ_TMA also the TMA'd P tile); sQ: the TMA'd Q tile
   double* sP = reinterpret_cast<double*>(tiles + Cfg::P_OFF);
-  double* sP2 = Cfg::PQ_TMA ? sP : reinterpret_cast<double*>(tiles);   // (per-thread slots; the parking is over by then)
-  double* sQ = Cfg::PQ_TMA ? reinterpret_cast<double*>(tiles + Cfg::Q_OFF)
-                           : reinterpret_cast<double*>(tiles) + NF * Cfg::THREADS;
-  static_assert(Cfg::PQ_TMA || Cfg::NSTAGE * Cfg::STAGE_BYTES >= 2 * NF * Cfg::THREADS * 8, "ring too small");
+  double* sQ = reinterpret_cast<double*>(tiles + Cfg::Q_OFF);
   int* lists = reinterpret_cast<int*>(tiles + Cfg::LIST_OFF);
   const int tid = threadIdx.x;
   const int lx = tid % Cfg::TX, ly = (tid / Cfg::TX) % Cfg::TY, lz = tid / (Cfg::TX * Cfg::TY);
@@ -272,7 +273,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 #pragma unroll
     for (int f = 0; f < NF; ++f) out[f] = 0.0;
     Geom G;
-    if (PARK) {
+    if (Cfg::EARLY_PARK) {
+      double* slot = reinterpret_cast<double*>(tiles + Cfg::E_OFF) + tid;
+      asm volatile("" ::: "memory");
+      geometry(u, D, G);
+      asm volatile("" ::: "memory");
+      park_late_derivs<false>(D, slot, Cfg::THREADS);
+    } else if (PARK) {
       // the tile ring is idle now: park what only the final assembly reads while geometry() peaks
       // (this thread's last stencil loads are complete -- their values were consumed above -- and no TMA is
       // pending; other threads' reads of the ring are fenced by the barrier above)
@@ -305,20 +312,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   if (STAGE >= 2 && Cfg::PQ_TMA) mbar_wait(pqbar, 0);
   if (active) {
     double* qc = sa.Q + ci;
-    if (!Cfg::PQ_TMA) {
-      // all loads of the RK registers first, as one batch of independent requests, parked in the (now idle) tile
-      // ring at the slots the code below reads (the stores to P/Q may alias the loads as far as the compiler knows)
-      double Pold[NF], Qold[NF];
+    // without PQ_TMA: all loads of the RK registers first, as one batch of independent requests (the stores to P/Q
+    // below may alias the loads as far as the compiler knows, which would otherwise serialise them)
+    double Pold[NF], Qold[NF];
 #pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        Qold[f] = STAGE >= 2 ? __ldcg(qc + f * g.is) : 0.0;
-        Pold[f] = STAGE >= 3 ? __ldcg(pc + f * g.is) : 0.0;
-      }
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        sQ[f * Cfg::THREADS + tid] = Qold[f];
-        if (STAGE >= 3) sP2[f * Cfg::THREADS + tid] = Pold[f];
-      }
+    for (int f = 0; f < NF; ++f) {
+      Qold[f] = (!Cfg::PQ_TMA && STAGE >= 2) ? __ldcg(qc + f * g.is) : 0.0;
+      Pold[f] = (!Cfg::PQ_TMA && STAGE >= 3) ? __ldcg(pc + f * g.is) : 0.0;
     }
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
@@ -328,19 +328,19 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
         u[f] = u[f] + 0.5 * P;
       } else if (STAGE == 2) {
         const double P = dt * out[f];
-        const double Q = sQ[f * Cfg::THREADS + tid];
+        const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
         pc[f * g.is] = P;
         u[f] = u[f] + 0.5 * (P - Q);
         qc[f * g.is] = Q / 6.0;
       } else if (STAGE == 3) {
-        const double P = -0.5 * sP2[f * Cfg::THREADS + tid] + dt * out[f];
-        const double Q = sQ[f * Cfg::THREADS + tid];
+        const double P = -0.5 * (Cfg::PQ_TMA ? sP[f * Cfg::THREADS + tid] : Pold[f]) + dt * out[f];
+        const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
         pc[f * g.is] = P;
         u[f] = u[f] + P;
         qc[f * g.is] = Q - P;
       } else {
-        const double P = 2.0 * sP2[f * Cfg::THREADS + tid] + dt * out[f];
-        const double Q = sQ[f * Cfg::THREADS + tid];
+        const double P = 2.0 * (Cfg::PQ_TMA ? sP[f * Cfg::THREADS + tid] : Pold[f]) + dt * out[f];
+        const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
         u[f] = u[f] + (Q + P / 6.0);
       }
     }
@@ -377,7 +377,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
 using RhsTile2 = TileCfg<16, 4, 4, 3, 1>;
-using RhsTile5 = TileCfg<16, 4, 2, 5, 2, false>;   // 5-deep ring, P/Q by batched global loads (variant 4)
+// variant 4: P/Q by batched global loads + early parking. Measured 0.189 ms per launch at 64^3 against 0.183 ms for the
+// default; with the freed shared memory spent on a 5-deep ring instead it was 0.187 ms: neither the late tiles nor the
+// register pressure of the field stream is what limits the default kernel.
+using RhsTile5 = TileCfg<16, 4, 2, 3, 2, false>;
 
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 

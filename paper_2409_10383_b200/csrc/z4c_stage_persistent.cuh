@@ -34,6 +34,8 @@ struct PersistCfg {
   static constexpr int LIST_OFF = B_OFF + NPARK * THREADS * 8;
   static constexpr int MAXLIST = 32;
   static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
+  static constexpr bool EARLY_PARK = false;                   // (members field_from_tile looks at)
+  static constexpr int S_OFF = A_OFF, E_OFF = B_OFF;
   static_assert(NSTAGE >= 3, "the three shift components are staged together");
 };
 

@@ -133,7 +133,7 @@ def test_one_step_parity(Z, oracle, name):
     S = perturbation_scale(ref, p)
     results = []
     for kw in ({"variant": 0, "fused": 2}, {"variant": 1, "fused": 0}, {"variant": 0, "fused": 2, "graph": True},
-               {"variant": 0, "fused": 1}, {"variant": 3, "fused": 2}, {"variant": 2, "fused": 2}):   # 3 = persistent kernel
+               {"variant": 0, "fused": 1}, {"variant": 3, "fused": 2}, {"variant": 2, "fused": 2}, {"variant": 4, "fused": 2}):   # 3 = persistent kernel
         sim = make(Z, p, u, **kw)
         sim.step(1)
         sim.sync()
