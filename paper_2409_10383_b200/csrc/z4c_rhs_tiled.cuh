@@ -213,25 +213,33 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
       tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
       if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
     }
-    // push lists (O2): per axis, every (source cell of this tile -> destination block, padded index) pair,
-    // the cell's own position included; the destinations of the tile are the product of the three lists
-    if (STAGE >= 1) {
-      int bxyz[3];
-      block_coords(g, b, bxyz[0], bxyz[1], bxyz[2]);
-      const int c0[3] = {cx, cy, cz}, T[3] = {Cfg::TX, Cfg::TY, Cfg::TZ};
-      for (int a = 0; a < 3; ++a) {
-        int* L = lists + a * 3 * Cfg::MAXLIST;
-        int cnt = 0;
-        for (int l = c0[a]; l < c0[a] + T[a] && l < g.n; ++l) {
-          int tb[4], tl[4];
-          const int nt = push_targets(l, bxyz[a], g.n, g.nb[a], g.bc, tb, tl);
-          for (int q = 0; q < nt; ++q) {
-            L[cnt] = l - c0[a]; L[Cfg::MAXLIST + cnt] = tb[q]; L[2 * Cfg::MAXLIST + cnt] = tl[q];
-            ++cnt;
-          }
-        }
-        lists[9 * Cfg::MAXLIST + a] = cnt;
+  }
+  // push lists (O2): per axis, every (source cell of this tile -> destination block, padded index) pair, the
+  // cell's own position included; the destinations of the tile are the product of the three lists. Built by the
+  // LAST warp, one lane per source cell with a warp prefix sum for the list positions: a few dozen instructions,
+  // so that no warp arrives late at the first barrier (a serial build by thread 0 cost ~1 us per CTA).
+  if (STAGE >= 1 && tid >= Cfg::THREADS - 32) {
+    const int lane = tid & 31;
+    int bxyz[3];
+    block_coords(g, b, bxyz[0], bxyz[1], bxyz[2]);
+    const int c0[3] = {cx, cy, cz}, T[3] = {Cfg::TX, Cfg::TY, Cfg::TZ};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      int* L = lists + a * 3 * Cfg::MAXLIST;
+      const int l = c0[a] + lane;
+      int tb[4], tl[4];
+      const int nt = (lane < T[a] && l < g.n) ? push_targets(l, bxyz[a], g.n, g.nb[a], g.bc, tb, tl) : 0;
+      int incl = nt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += up;
       }
+      const int pos = incl - nt;
+      for (int q = 0; q < nt; ++q) {
+        L[pos + q] = lane; L[Cfg::MAXLIST + pos + q] = tb[q]; L[2 * Cfg::MAXLIST + pos + q] = tl[q];
+      }
+      if (lane == 31) lists[9 * Cfg::MAXLIST + a] = incl;
     }
   }
   const int toff = (lz + NG) * Cfg::SZ + (ly + NG) * Cfg::SY + lx + NG;
