@@ -366,8 +366,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   const int* Lz = lists + 6 * Cfg::MAXLIST;
   const int ncx = lists[9 * Cfg::MAXLIST], ncy = lists[9 * Cfg::MAXLIST + 1], ncz = lists[9 * Cfg::MAXLIST + 2];
   const int total = ncx * ncy * ncz;
+  // q -> (qx, qy, qz) with reciprocal multiplies: exact for these small ranges (q < 2^11, divisors <= 22: the
+  // quotient's fractional part stays >= 0.5/22 away from an integer, float error is ~1e-4 of that)
+  const float rcx = 1.0f / (float)ncx, rcy = 1.0f / (float)ncy;
   for (int q = tid; q < total; q += Cfg::THREADS) {
-    const int qx = q % ncx, r = q / ncx, qy = r % ncy, qz = r / ncy;
+    const int r = (int)(((float)q + 0.5f) * rcx), qx = q - r * ncx;
+    const int qz = (int)(((float)r + 0.5f) * rcy), qy = r - qz * ncy;
     const int src = (Lz[qz] * Cfg::TY + Ly[qy]) * Cfg::TX + Lx[qx];
     const long long tb = ((long long)Lz[Cfg::MAXLIST + qz] * g.nb[1] + Ly[Cfg::MAXLIST + qy]) * g.nb[0] + Lx[Cfg::MAXLIST + qx];
     double* d = sa.y_out + tb * g.m3 +
