@@ -22,7 +22,7 @@ class _OParams(C.Structure):
                 ("kappa1", C.c_double), ("kappa2", C.c_double),
                 ("lapse_oplog", C.c_double), ("lapse_harmonic", C.c_double), ("lapse_advect", C.c_double),
                 ("shift_gamma", C.c_double), ("shift_eta", C.c_double), ("shift_advect", C.c_double),
-                ("ko_eps", C.c_double), ("chi_floor", C.c_double)]
+                ("ko_eps", C.c_double), ("chi_floor", C.c_double), ("ng", C.c_int32)]
 
 
 def build(force: bool = False) -> str:
@@ -73,6 +73,7 @@ def _op(p, N=None) -> _OParams:
     for a in range(3):
         o.N[a] = int(NN[a])
     o.bc = int(p.bc)
+    o.ng = int(getattr(p, "ng", 3))      # 3 -> 4th-order stencils, 4 -> 6th-order (NEXT-1)
     for name in ("dx", "cfl", "kappa1", "kappa2", "lapse_oplog", "lapse_harmonic", "lapse_advect",
                  "shift_gamma", "shift_eta", "shift_advect", "ko_eps", "chi_floor"):
         setattr(o, name, float(getattr(p, name)))

@@ -61,24 +61,25 @@ static void gather(const View& V, int i, int j, int k, bool all_d1, T* u, Derivs
   const int c[3] = {i, j, k};
   for (int f = 0; f < NF; ++f) u[f] = T(V.at(f, i, j, k));
   for (int f = 0; f < NF; ++f) {
-    T line[3][7];
+    const bool o6 = sixth_order(V.P);
+    T line[3][9];
     for (int a = 0; a < 3; ++a)
-      for (int s = -3; s <= 3; ++s) {
+      for (int s = -4; s <= 4; ++s) {
         int q[3] = {c[0], c[1], c[2]};
         q[a] += s;
-        line[a][s + 3] = T(V.at(f, q[0], q[1], q[2]));
+        line[a][s + 4] = T(V.at(f, q[0], q[1], q[2]));
       }
     T adv = T(0.0), ko = T(0.0);
     for (int a = 0; a < 3; ++a) {
-      const T* l = &line[a][3];
-      if (NEEDS_D1[f] || all_d1) D.d1[f][a] = d1_centred(l, h); else D.d1[f][a] = T(0.0);
-      if (NEEDS_D2[f]) D.d2[f][SYM[a][a]] = d2_centred(l, h);
+      const T* l = &line[a][4];
+      if (NEEDS_D1[f] || all_d1) D.d1[f][a] = o6 ? d1_centred6(l, h) : d1_centred(l, h); else D.d1[f][a] = T(0.0);
+      if (NEEDS_D2[f]) D.d2[f][SYM[a][a]] = o6 ? d2_centred6(l, h) : d2_centred(l, h);
       const T beta = u[BETAX + a];
-      adv = adv + beta * d1_upwind(l, h, value(beta) >= 0.0);
-      ko = ko + ko_axis(l);
+      adv = adv + beta * (o6 ? d1_upwind6(l, h, value(beta) >= 0.0) : d1_upwind(l, h, value(beta) >= 0.0));
+      ko = ko + (o6 ? ko_axis6(l) : ko_axis(l));
     }
     D.adv[f] = adv;
-    D.ko[f] = T(V.P.ko_eps / (64.0 * h)) * ko;
+    D.ko[f] = T(V.P.ko_eps / ((o6 ? 256.0 : 64.0) * h)) * ko;
     if (NEEDS_D2[f]) {
       for (int a = 0; a < 3; ++a)
         for (int b = a + 1; b < 3; ++b) {
@@ -87,7 +88,7 @@ static void gather(const View& V, int i, int j, int k, bool all_d1, T* u, Derivs
             q[a] += sa; q[b] += sb;
             return T(V.at(f, q[0], q[1], q[2]));
           };
-          D.d2[f][SYM[a][b]] = d2_mixed<T>(v, h);
+          D.d2[f][SYM[a][b]] = o6 ? d2_mixed6<T>(v, h) : d2_mixed<T>(v, h);
         }
     } else {
       for (int p = 0; p < 6; ++p) D.d2[f][p] = T(0.0);
@@ -316,27 +317,31 @@ void oz4c_stencil(const Params* P, const double* f, int kind, int a, int b, doub
     for (int j = 0; j < P->N[1]; ++j)
       for (int i = 0; i < P->N[0]; ++i) {
         const int c[3] = {i, j, k};
+        const bool o6 = sixth_order(*P);
         auto line = [&](int ax, double* l) {
-          for (int s = -3; s <= 3; ++s) {
+          for (int s = -4; s <= 4; ++s) {
             int q[3] = {c[0], c[1], c[2]};
             q[ax] += s;
-            l[s + 3] = V.at(0, q[0], q[1], q[2]);
+            l[s + 4] = V.at(0, q[0], q[1], q[2]);
           }
         };
-        double l[7], r = 0.0;
-        if (kind == 0) { line(a, l); r = d1_centred(&l[3], h); }
-        else if (kind == 1) { line(a, l); r = d2_centred(&l[3], h); }
+        double lbuf[9], r = 0.0;
+        double* l = lbuf + 1;   // so that &l[3] is the centre in both layouts
+        if (kind == 0) { line(a, lbuf); r = o6 ? d1_centred6(&l[3], h) : d1_centred(&l[3], h); }
+        else if (kind == 1) { line(a, lbuf); r = o6 ? d2_centred6(&l[3], h) : d2_centred(&l[3], h); }
         else if (kind == 2) {
           auto v = [&](int sa, int sb) -> double {
             int q[3] = {c[0], c[1], c[2]};
             q[a] += sa; q[b] += sb;
             return V.at(0, q[0], q[1], q[2]);
           };
-          r = d2_mixed<double>(v, h);
-        } else if (kind == 3 || kind == 4) { line(a, l); r = d1_upwind(&l[3], h, kind == 3); }
-        else {
-          for (int ax = 0; ax < 3; ++ax) { line(ax, l); r += ko_axis(&l[3]); }
-          r *= P->ko_eps / (64.0 * h);
+          r = o6 ? d2_mixed6<double>(v, h) : d2_mixed<double>(v, h);
+        } else if (kind == 3 || kind == 4) {
+          line(a, lbuf);
+          r = o6 ? d1_upwind6(&l[3], h, kind == 3) : d1_upwind(&l[3], h, kind == 3);
+        } else {
+          for (int ax = 0; ax < 3; ++ax) { line(ax, lbuf); r += o6 ? ko_axis6(&l[3]) : ko_axis(&l[3]); }
+          r *= P->ko_eps / ((o6 ? 256.0 : 64.0) * h);
         }
         out[((size_t)k * P->N[1] + j) * P->N[0] + i] = r;
       }

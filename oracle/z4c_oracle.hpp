@@ -44,7 +44,10 @@ struct Params {
   double shift_gamma, shift_eta, shift_advect;
   double ko_eps;        // PAPER.md:203 (0.5)
   double chi_floor;     // Q8
+  int32_t ng;           // ghost zones of the GPU layout = stencil half-width: 3 (or 0) -> 4th order (Q1),
+                        // 4 -> 6th order, the paper's production scheme ("6th order with 4 ghosts", 279)
 };
+inline bool sixth_order(const Params& P) { return P.ng == 4; }
 
 // ---------------------------------------------------------------------------------
 // O3 stencils, all in difference-from-centre form (Q14).  `l` points at the centre of
@@ -91,6 +94,50 @@ inline T d2_mixed(V v, double h) {
     inner[sb + 2] = T(8.0) * (v(1, sb) - v(-1, sb)) - (v(2, sb) - v(-2, sb));
   }
   return (T(8.0) * (inner[3] - inner[1]) - (inner[4] - inner[0])) / T(144.0 * h * h);
+}
+
+// ---------------------------------------------------------------------------------
+// NEXT-1: the 6th-order set for 4 ghost zones (PAPER.md:124 footnote: "6th order with 4 ghosts";
+// the scheme of every performance run). Coefficients are the unique ones of their
+// support and order (pinned by polynomial exactness to degree 6 in tests/test_oracle_pins.py):
+//   centred 1st  (-1, 9, -45, 0, 45, -9, 1)/60;  centred 2nd (2, -27, 270, -490, 270, -27, 2)/180;
+//   lopsided 1st on offsets -2..+4: (2, -24, -35, 80, -30, 8, -1)/60 (mirror, sign flipped, for beta < 0);
+//   Kreiss-Oliger: -eps h^7/256 d^8 (9 points), i.e. (eps/256h)(56 s1 - 28 s2 + 8 s3 - s4), s_k = d_k + d_-k.
+// Same difference-from-centre form as above (Q14).
+// ---------------------------------------------------------------------------------
+template <class T>
+inline T d1_centred6(const T* l, double h) {
+  return (T(45.0) * (l[1] - l[-1]) - T(9.0) * (l[2] - l[-2]) + (l[3] - l[-3])) / T(60.0 * h);
+}
+template <class T>
+inline T d2_centred6(const T* l, double h) {
+  T s1 = (l[1] - l[0]) + (l[-1] - l[0]), s2 = (l[2] - l[0]) + (l[-2] - l[0]), s3 = (l[3] - l[0]) + (l[-3] - l[0]);
+  return (T(270.0) * s1 - T(27.0) * s2 + T(2.0) * s3) / T(180.0 * h * h);
+}
+template <class T>
+inline T d1_upwind6(const T* l, double h, bool positive) {
+  const int g = positive ? 1 : -1;   // mirror the offsets for beta < 0 and flip the sign
+  T dm2 = l[-2 * g] - l[0], dm1 = l[-g] - l[0], dp1 = l[g] - l[0], dp2 = l[2 * g] - l[0], dp3 = l[3 * g] - l[0],
+    dp4 = l[4 * g] - l[0];
+  T num = T(2.0) * dm2 - T(24.0) * dm1 + T(80.0) * dp1 - T(30.0) * dp2 + T(8.0) * dp3 - dp4;
+  return positive ? num / T(60.0 * h) : num / T(-60.0 * h);
+}
+template <class T>
+inline T ko_axis6(const T* l) {
+  // 56 s1 - 28 s2 + 8 s3 - s4; caller multiplies by eps/(256h)
+  T s1 = (l[1] - l[0]) + (l[-1] - l[0]), s2 = (l[2] - l[0]) + (l[-2] - l[0]);
+  T s3 = (l[3] - l[0]) + (l[-3] - l[0]), s4 = (l[4] - l[0]) + (l[-4] - l[0]);
+  return T(56.0) * s1 - T(28.0) * s2 + T(8.0) * s3 - s4;
+}
+template <class T, class V>
+inline T d2_mixed6(V v, double h) {
+  // centred-1st (6th order) along b of centred-1st along a; v(sa,sb) for sa,sb in {-3..3}\{0}
+  T inner[7];
+  for (int sb = -3; sb <= 3; ++sb) {
+    if (sb == 0) { inner[3] = T(0.0); continue; }
+    inner[sb + 3] = T(45.0) * (v(1, sb) - v(-1, sb)) - T(9.0) * (v(2, sb) - v(-2, sb)) + (v(3, sb) - v(-3, sb));
+  }
+  return (T(45.0) * (inner[4] - inner[2]) - T(9.0) * (inner[5] - inner[1]) + (inner[6] - inner[0])) / T(3600.0 * h * h);
 }
 
 // ---------------------------------------------------------------------------------

@@ -420,3 +420,91 @@ def test_flop_census(oracle):
     c2 = oracle.count_flops(p, u, 3, 4, 5)["rhs"]
     tot2 = c2["add"] + c2["mul"] + c2["div"]
     assert bench.RHS_FLOPS_PER_CELL <= tot2 <= bench.RHS_FLOPS_PER_CELL + 66 and c2["add"] == c["add"]
+
+
+# ---------------------------------------------------------------- NEXT-1: 6th-order stencil set (4 ghosts)
+def _poly_grid6(N=14, h=0.37):
+    p = replace(box_params(N, (-1.3, 0.4, 2.1), N * h, ko_eps=0.5), ng=4)
+    z, y, x = I.cell_centres(p)
+    return p, x + 0 * y + 0 * z, y + 0 * x + 0 * z, z + 0 * x + 0 * y
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_N1_sixth_order_stencils_exact_on_degree6(oracle, axis):
+    p, xx, yy, zz = _poly_grid6()
+    c = [xx, yy, zz][axis]
+    h = p.dx
+    for deg in range(0, 7):
+        f = c ** deg
+        d1 = deg * c ** max(deg - 1, 0)
+        d2 = deg * (deg - 1) * c ** max(deg - 2, 0)
+        scale = np.abs(inner(f, 4)).max() / h
+        for kind in (0, 3, 4):
+            err = np.abs(inner(oracle.stencil(p, f, kind, axis), 4) - inner(d1, 4)).max()
+            assert err <= 5e-13 * scale, (kind, deg, err)
+        err = np.abs(inner(oracle.stencil(p, f, 1, axis), 4) - inner(d2, 4)).max()
+        assert err <= 5e-13 * scale / h, (deg, err)
+    # the order-7 KO operator annihilates degree <= 7
+    f = c ** 7 - 2 * c ** 4
+    assert np.abs(inner(oracle.stencil(p, f, 5), 4)).max() <= 1e-10 * np.abs(f).max() / h
+
+
+def test_N1_sixth_order_leading_terms_mixed_and_ko_sign(oracle):
+    p, xx, yy, zz = _poly_grid6()
+    h = p.dx
+    # centred-1st: +h^6 u^(7)/140 ; lopsided: -h^6 u^(7)/105 on both sides ; KO = -eps h^7 u^(8)/256
+    f7 = xx ** 7
+    exact = 7 * xx ** 6
+    assert np.allclose(inner(oracle.stencil(p, f7, 0, 0), 4) - inner(exact, 4), h ** 6 * 5040 / 140, rtol=1e-6)
+    for kind in (3, 4):
+        assert np.allclose(inner(oracle.stencil(p, f7, kind, 0), 4) - inner(exact, 4), -h ** 6 * 5040 / 105, rtol=1e-6)
+    f8 = yy ** 8
+    assert np.allclose(inner(oracle.stencil(p, f8, 5), 4), -p.ko_eps * h ** 7 * 40320 / 256, rtol=1e-6)
+    # mixed derivative: exact on x^a y^b with a, b <= 6, and symmetric
+    c = [xx, yy, zz]
+    for a in range(3):
+        for b in range(a + 1, 3):
+            f = c[a] ** 6 * c[b] ** 5 + 2 * c[a] * c[b] ** 6
+            exact = 30 * c[a] ** 5 * c[b] ** 4 + 12 * c[b] ** 5
+            got = oracle.stencil(p, f, 2, a, b)
+            tol = 1e-11 * np.abs(f).max() / p.dx ** 2
+            assert np.abs(inner(got, 4) - inner(exact, 4)).max() <= tol
+            assert np.abs(inner(got, 4) - inner(oracle.stencil(p, f, 2, b, a), 4)).max() <= tol
+    # damping: the highest-frequency mode is opposed with symbol -eps sin^8(kh/2)/h
+    pn = replace(I.params_noise(8, (1, 1, 1), 0.1), ng=4)
+    i = np.arange(8)
+    f = np.broadcast_to(((-1.0) ** i)[None, None, :], (8, 8, 8)).copy()
+    assert np.allclose(oracle.stencil(pn, f, 5), -pn.ko_eps / pn.dx * f, rtol=1e-13)
+
+
+def test_N1_sixth_order_convergence_and_minkowski(oracle):
+    # Minkowski stays an exact fixed point
+    pm = replace(I.params_noise(10, (1, 1, 1)), ng=4)
+    assert np.all(oracle.rhs(pm, I.minkowski(pm)) == 0.0)
+    # static isotropic Schwarzschild: the metric-sector RHS converges to zero at 6th order (P4 at the new order)
+    errs = []
+    for N in (16, 32):
+        p = replace(box_params(N, (1.0, 1.2, 0.8), 2.0, ko_eps=0.0, lapse_oplog=2.0), ng=4)
+        z, y, x = I.cell_centres(p)
+        r = np.sqrt(x * x + y * y + z * z)
+        psi = 1.0 + 0.5 / r
+        u = I.minkowski(p)
+        u[I.CHI] = psi ** -4
+        u[I.ALPHA] = (1.0 - 0.5 / r) / psi
+        rhs = oracle.rhs(p, u)
+        m = N // 4
+        errs.append(np.abs(inner(rhs[I.AXX:I.AZZ + 1], m)).max())
+    assert errs[1] < errs[0] / 40.0, errs          # 2^6 = 64 asymptotically
+    # linear wave: one period fraction at 6th order beats 4th order by a wide margin at the same resolution
+    p4 = I.params_linear_wave(32, 16)
+    p6 = replace(p4, ng=4)
+    u0 = I.linear_wave_data(p4)
+    pen = lambda p: replace(p, nb=(2, 1, 1), n=16)   # noqa: E731  (x-pencil 32 x 16 x 16, same data along x)
+    up = np.ascontiguousarray(u0[:, :16, :16, :])
+    e = {}
+    for name, pp in (("o4", pen(p4)), ("o6", pen(p6))):
+        out, bad = oracle.step(pp, oracle.enforce(pp, up)[0], 16)
+        assert bad == 0
+        exact = I.linear_wave_data(pp, t=16 * pp.dt)
+        e[name] = np.abs(out[I.GYY] - exact[I.GYY]).max()
+    assert e["o6"] < e["o4"] / 5.0, e
