@@ -40,13 +40,14 @@ __global__ void __launch_bounds__(256) k_layout(Pack g, double* __restrict__ pac
 // ---------------------------------------------------------------------------------------------
 // K1 same-level ghost fill (S1). One thread per (ghost cell, block); it moves all 22 fields of that
 // cell (22 independent 8-byte copies in flight). Ghost cells are enumerated shell by shell so no thread
-// is idle: z-slabs (6 m^2 cells), y-slabs (6 n m), x-slabs (6 n^2).
+// is idle: z-slabs (2 NG m^2 cells), y-slabs (2 NG n m), x-slabs (2 NG n^2).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int ghost_coord(int q, int n) { return q < NG ? q : n + q; }  // q in [0,6)
+__device__ __forceinline__ int ghost_coord(int q, int n) { return q < NG ? q : n + q; }  // q in [0, 2 NG)
 
 __global__ void __launch_bounds__(256) k_ghost_fill(Pack g, double* __restrict__ y) {
   const int n = g.n, m = g.m;
-  const int nZ = 6 * m * m, nY = 6 * n * m, nX = 6 * n * n;
+  constexpr int G2 = 2 * NG;
+  const int nZ = G2 * m * m, nY = G2 * n * m, nX = G2 * n * n;
   const int per_block = nZ + nY + nX;
   const long long total = (long long)per_block * g.nblk;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
@@ -58,10 +59,10 @@ __global__ void __launch_bounds__(256) k_ghost_fill(Pack g, double* __restrict__
       i = r % m; j = (r / m) % m; k = ghost_coord(r / (m * m), n);
     } else if (r < nZ + nY) {
       r -= nZ;
-      i = r % m; j = ghost_coord((r / m) % 6, n); k = NG + r / (6 * m);
+      i = r % m; j = ghost_coord((r / m) % G2, n); k = NG + r / (G2 * m);
     } else {
       r -= nZ + nY;
-      i = ghost_coord(r % 6, n); j = NG + (r / 6) % n; k = NG + r / (6 * n);
+      i = ghost_coord(r % G2, n); j = NG + (r / G2) % n; k = NG + r / (G2 * n);
     }
     int bx, by, bz;
     block_coords(g, b, bx, by, bz);
@@ -278,7 +279,7 @@ __global__ void __launch_bounds__(128) k_stage_update(Pack g, double* __restrict
     if (edge) {
       int bx, by, bz;
       block_coords(g, b, bx, by, bz);
-      int tbx[4], tlx[4], tby[4], tly[4], tbz[4], tlz[4];
+      int tbx[NG + 1], tlx[NG + 1], tby[NG + 1], tly[NG + 1], tbz[NG + 1], tlz[NG + 1];
       const int cx = push_targets(i, bx, g.n, g.nb[0], g.bc, tbx, tlx);
       const int cy = push_targets(j, by, g.n, g.nb[1], g.bc, tby, tly);
       const int cz = push_targets(k, bz, g.n, g.nb[2], g.bc, tbz, tlz);

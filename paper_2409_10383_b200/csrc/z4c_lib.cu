@@ -103,7 +103,7 @@ int grid_for(long long total, int threads, long long cap = (1LL << 30)) {
 
 // ---- launch helpers (all asynchronous on c->stream) ---------------------------------------
 int launch_ghost_fill(z4c_ctx* c) {
-  const long long per_block = 6LL * c->g.m * c->g.m + 6LL * c->g.n * c->g.m + 6LL * c->g.n * c->g.n;
+  const long long per_block = 2LL * NG * ((long long)c->g.m * c->g.m + (long long)c->g.n * c->g.m + (long long)c->g.n * c->g.n);
   k_ghost_fill<<<grid_for(per_block * c->g.nblk, 256), 256, 0, c->stream>>>(c->g, c->y);
   return check_launch(c, "k_ghost_fill");
 }
@@ -303,10 +303,17 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->prm = *p;
   c->g = make_pack(*p);
   const double h = p->dx;
-  c->fd.inv12h = 1.0 / (12.0 * h);
-  c->fd.inv12h2 = 1.0 / (12.0 * h * h);
-  c->fd.inv144h2 = 1.0 / (144.0 * h * h);
-  c->fd.ko = p->ko_eps / (64.0 * h);
+  if (NG == 3) {   // 4th-order set (O3)
+    c->fd.inv12h = 1.0 / (12.0 * h);
+    c->fd.inv12h2 = 1.0 / (12.0 * h * h);
+    c->fd.inv144h2 = 1.0 / (144.0 * h * h);
+    c->fd.ko = p->ko_eps / (64.0 * h);
+  } else {         // 6th-order set (NEXT-1)
+    c->fd.inv12h = 1.0 / (60.0 * h);
+    c->fd.inv12h2 = 1.0 / (180.0 * h * h);
+    c->fd.inv144h2 = 1.0 / (3600.0 * h * h);
+    c->fd.ko = p->ko_eps / (256.0 * h);
+  }
   c->sp.kappa1 = p->kappa1; c->sp.kappa2 = p->kappa2;
   c->sp.lapse_oplog = p->lapse_oplog; c->sp.lapse_harmonic = p->lapse_harmonic; c->sp.lapse_advect = p->lapse_advect;
   c->sp.shift_gamma = p->shift_gamma; c->sp.shift_eta = p->shift_eta; c->sp.shift_advect = p->shift_advect;

@@ -13,7 +13,14 @@ enum : int {
   AXX = 8, AXY = 9, AXZ = 10, AYY = 11, AYZ = 12, AZZ = 13,
   GAMX = 14, GAMY = 15, GAMZ = 16, THETA = 17, ALPHA = 18, BETAX = 19, BETAY = 20, BETAZ = 21
 };
-constexpr int NG = 3;
+// Ghost zones per side = stencil half-width, fixed at compile time: 3 -> 4th-order stencils (BASELINE configs),
+// 4 -> 6th-order stencils, the paper's production scheme (NEXT-1). The library is built once
+// per value (libz4c.so, libz4c_ng4.so).
+#ifndef Z4C_NG
+#define Z4C_NG 3
+#endif
+constexpr int NG = Z4C_NG;
+static_assert(NG == 3 || NG == 4, "supported ghost counts");
 
 // packed index of a symmetric pair: xx,xy,xz,yy,yz,zz
 __host__ __device__ constexpr int sym(int i, int j) {
@@ -21,11 +28,12 @@ __host__ __device__ constexpr int sym(int i, int j) {
 }
 
 // Per-launch constants of the finite-difference operators.
+// (NG = 3 values; NG = 4 in brackets)
 struct FdConst {
-  double inv12h;     // 1/(12 h)
-  double inv12h2;    // 1/(12 h^2)
-  double inv144h2;   // 1/(144 h^2)
-  double ko;         // eps/(64 h)
+  double inv12h;     // 1/(12 h)      [1/(60 h)]    centred 1st; half of it weights the upwinded term
+  double inv12h2;    // 1/(12 h^2)    [1/(180 h^2)] centred 2nd
+  double inv144h2;   // 1/(144 h^2)   [1/(3600 h^2)] mixed 2nd
+  double ko;         // eps/(64 h)    [eps/(256 h)] Kreiss-Oliger
 };
 
 // One axis of one field: 6 neighbour loads feed the centred 1st/2nd derivative, the upwinded
@@ -36,10 +44,11 @@ struct AxisRaw { double d1, d2, up, ko; };
 template <bool WANT_D1, bool WANT_D2>
 __device__ __forceinline__ AxisRaw axis_raw(const double* __restrict__ p, const int s, const double c,
                                             const bool pos) {
+  AxisRaw r;
+#if Z4C_NG == 3
   const double lm3 = __ldg(p - 3 * s), lm2 = __ldg(p - 2 * s), lm1 = __ldg(p - s);
   const double lp1 = __ldg(p + s), lp2 = __ldg(p + 2 * s), lp3 = __ldg(p + 3 * s);
   const double dm1 = lm1 - c, dp1 = lp1 - c, dm2 = lm2 - c, dp2 = lp2 - c, dm3 = lm3 - c, dp3 = lp3 - c;
-  AxisRaw r;
   const double s1 = dp1 + dm1, s2 = dp2 + dm2, s3 = dp3 + dm3;
   r.d1 = WANT_D1 ? (8.0 * (lp1 - lm1) - (lp2 - lm2)) : 0.0;
   r.d2 = WANT_D2 ? (16.0 * s1 - s2) : 0.0;
@@ -49,20 +58,43 @@ __device__ __forceinline__ AxisRaw axis_raw(const double* __restrict__ p, const 
   const double a1 = pos ? dp1 : dm1, b1 = pos ? dm1 : dp1;
   const double a2 = pos ? dp2 : dm2, a3 = pos ? dp3 : dm3;
   r.up = -3.0 * b1 + 18.0 * a1 - 6.0 * a2 + a3;
+#else
+  // 6th order: centred (45 e1 - 9 e2 + e3)/60h, (270 s1 - 27 s2 + 2 s3)/180h^2; KO (56 s1 - 28 s2 + 8 s3 - s4);
+  // lopsided numerator on the upwind side, offsets -2..+4: 2 d-2 - 24 d-1 + 80 d+1 - 30 d+2 + 8 d+3 - d+4
+  const double lm4 = __ldg(p - 4 * s), lm3 = __ldg(p - 3 * s), lm2 = __ldg(p - 2 * s), lm1 = __ldg(p - s);
+  const double lp1 = __ldg(p + s), lp2 = __ldg(p + 2 * s), lp3 = __ldg(p + 3 * s), lp4 = __ldg(p + 4 * s);
+  const double dm1 = lm1 - c, dp1 = lp1 - c, dm2 = lm2 - c, dp2 = lp2 - c, dm3 = lm3 - c, dp3 = lp3 - c,
+               dm4 = lm4 - c, dp4 = lp4 - c;
+  const double s1 = dp1 + dm1, s2 = dp2 + dm2, s3 = dp3 + dm3, s4 = dp4 + dm4;
+  r.d1 = WANT_D1 ? (45.0 * (lp1 - lm1) - 9.0 * (lp2 - lm2) + (lp3 - lm3)) : 0.0;
+  r.d2 = WANT_D2 ? (270.0 * s1 - 27.0 * s2 + 2.0 * s3) : 0.0;
+  r.ko = 56.0 * s1 - 28.0 * s2 + 8.0 * s3 - s4;
+  const double b2 = pos ? dm2 : dp2, b1 = pos ? dm1 : dp1;
+  const double a1 = pos ? dp1 : dm1, a2 = pos ? dp2 : dm2, a3 = pos ? dp3 : dm3, a4 = pos ? dp4 : dm4;
+  r.up = 2.0 * b2 - 24.0 * b1 + 80.0 * a1 - 30.0 * a2 + 8.0 * a3 - a4;
+#endif
   return r;
 }
 
 // centred 1st derivative only (fields/axes where nothing else is needed: K4's d_k At_ij)
 __device__ __forceinline__ double d1_raw(const double* __restrict__ p, const int s) {
+#if Z4C_NG == 3
   return 8.0 * (__ldg(p + s) - __ldg(p - s)) - (__ldg(p + 2 * s) - __ldg(p - 2 * s));
+#else
+  return 45.0 * (__ldg(p + s) - __ldg(p - s)) - 9.0 * (__ldg(p + 2 * s) - __ldg(p - 2 * s)) +
+         (__ldg(p + 3 * s) - __ldg(p - 3 * s));
+#endif
 }
 
-// mixed second derivative D_b(D_a u), raw (scale 1/(144 h^2)); 16 loads
+// mixed second derivative D_b(D_a u), raw (scale 1/(144 h^2) [1/(3600 h^2)]); 16 [36] loads
 __device__ __forceinline__ double mixed_raw(const double* __restrict__ p, const int sa, const int sb) {
-  auto inner = [&](const double* q) {
-    return 8.0 * (__ldg(q + sa) - __ldg(q - sa)) - (__ldg(q + 2 * sa) - __ldg(q - 2 * sa));
-  };
+  auto inner = [&](const double* q) { return d1_raw(q, sa); };
+#if Z4C_NG == 3
   return 8.0 * (inner(p + sb) - inner(p - sb)) - (inner(p + 2 * sb) - inner(p - 2 * sb));
+#else
+  return 45.0 * (inner(p + sb) - inner(p - sb)) - 9.0 * (inner(p + 2 * sb) - inner(p - 2 * sb)) +
+         (inner(p + 3 * sb) - inner(p - 3 * sb));
+#endif
 }
 
 // ---- 3x3 symmetric algebra ------------------------------------------------------------------

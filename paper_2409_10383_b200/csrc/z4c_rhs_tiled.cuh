@@ -52,7 +52,7 @@ __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* m
 // PQ_TMA_: true = the CTA's P/Q register tiles are TMA-prefetched into shared memory at kernel start;
 // false = they are read in the epilogue as one batch of independent global loads (lines requested into L2 by a
 // prefetch at kernel start), which frees 2 x 22 x THREADS x 8 bytes of shared memory for a deeper tile ring.
-template <int TX_, int TY_, int TZ_, int NSTAGE_, int MINB_ = 1, bool PQ_TMA_ = true>
+template <int TX_, int TY_, int TZ_, int NSTAGE_, int MINB_ = 1, bool PQ_TMA_ = true, bool EARLY_PARK_ = !PQ_TMA_>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NSTAGE = NSTAGE_, MINB = MINB_;
   static constexpr bool PQ_TMA = PQ_TMA_;
@@ -70,7 +70,7 @@ struct TileCfg {
   static constexpr int S_OFF = Q_OFF + (PQ_TMA ? REG_BYTES : 0);
   // without PQ_TMA the freed space holds a dedicated parking area for the late-use derivatives (written as each
   // field is done, so they stay out of registers through the whole field stream)
-  static constexpr bool EARLY_PARK = !PQ_TMA;
+  static constexpr bool EARLY_PARK = EARLY_PARK_;
   static constexpr int E_OFF = S_OFF + REG_BYTES;
   static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0);   // push lists
   static constexpr int MAXLIST = 32;
@@ -86,6 +86,7 @@ __host__ __device__ constexpr int stream_field(int it) { return it < 3 ? BETAX +
 template <int S, bool WANT_D1, bool WANT_D2>
 __device__ __forceinline__ void axis_tile(const double* t, const double c, const double bw, const double aw,
                                           const FdConst& fd, double& d1, double& d2, double& adv, double& ko) {
+#if Z4C_NG == 3
   const double lm3 = t[-3 * S], lm2 = t[-2 * S], lm1 = t[-S], lp1 = t[S], lp2 = t[2 * S], lp3 = t[3 * S];
   const double e1 = lp1 - lm1, e2 = lp2 - lm2, e3 = lp3 - lm3;
   const double s1 = (lp1 - c) + (lm1 - c), s2 = (lp2 - c) + (lm2 - c), s3 = (lp3 - c) + (lm3 - c);
@@ -93,6 +94,19 @@ __device__ __forceinline__ void axis_tile(const double* t, const double c, const
   if (WANT_D2) d2 = (16.0 * s1 - s2) * fd.inv12h2;
   const double k = s3 - 6.0 * s2 + 15.0 * s1;
   const double sy = e3 - 6.0 * e2 + 21.0 * e1;
+#else
+  // 6th order (NEXT-1). The lopsided pair obeys the same identity as at 4th order:
+  //   D^+ + D^- = (104 e1 - 32 e2 + 8 e3 - e4)/(60h),   D^+ - D^- = (56 s1 - 28 s2 + 8 s3 - s4)/(60h) = KO sum/(60h)
+  const double lm4 = t[-4 * S], lm3 = t[-3 * S], lm2 = t[-2 * S], lm1 = t[-S];
+  const double lp1 = t[S], lp2 = t[2 * S], lp3 = t[3 * S], lp4 = t[4 * S];
+  const double e1 = lp1 - lm1, e2 = lp2 - lm2, e3 = lp3 - lm3, e4 = lp4 - lm4;
+  const double s1 = (lp1 - c) + (lm1 - c), s2 = (lp2 - c) + (lm2 - c), s3 = (lp3 - c) + (lm3 - c),
+               s4 = (lp4 - c) + (lm4 - c);
+  if (WANT_D1) d1 = (45.0 * e1 - 9.0 * e2 + e3) * fd.inv12h;
+  if (WANT_D2) d2 = (270.0 * s1 - 27.0 * s2 + 2.0 * s3) * fd.inv12h2;
+  const double k = 56.0 * s1 - 28.0 * s2 + 8.0 * s3 - s4;
+  const double sy = 104.0 * e1 - 32.0 * e2 + 8.0 * e3 - e4;
+#endif
   adv += bw * sy + aw * k;
   ko += k;
 }
@@ -100,8 +114,16 @@ __device__ __forceinline__ void axis_tile(const double* t, const double c, const
 // mixed second derivative from the tile, compile-time strides
 template <int SA, int SB>
 __device__ __forceinline__ double mixed_tile(const double* t) {
+#if Z4C_NG == 3
   auto inner = [&](const double* q) { return 8.0 * (q[SA] - q[-SA]) - (q[2 * SA] - q[-2 * SA]); };
   return 8.0 * (inner(t + SB) - inner(t - SB)) - (inner(t + 2 * SB) - inner(t - 2 * SB));
+#else
+  auto inner = [&](const double* q) {
+    return 45.0 * (q[SA] - q[-SA]) - 9.0 * (q[2 * SA] - q[-2 * SA]) + (q[3 * SA] - q[-3 * SA]);
+  };
+  return 45.0 * (inner(t + SB) - inner(t - SB)) - 9.0 * (inner(t + 2 * SB) - inner(t - 2 * SB)) +
+         (inner(t + 3 * SB) - inner(t - 3 * SB));
+#endif
 }
 
 template <class Cfg, int F>
@@ -227,7 +249,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     for (int a = 0; a < 3; ++a) {
       int* L = lists + a * 3 * Cfg::MAXLIST;
       const int l = c0[a] + lane;
-      int tb[4], tl[4];
+      int tb[NG + 1], tl[NG + 1];
       const int nt = (lane < T[a] && l < g.n) ? push_targets(l, bxyz[a], g.n, g.nb[a], g.bc, tb, tl) : 0;
       int incl = nt;
 #pragma unroll
@@ -387,12 +409,23 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   64^3 wave: 0.202 ms per launch against 0.213 ms for the 16x4x4 tile (256 threads, 1 CTA per SM);
 //   256^3 two punctures: 9.94 against 10.76 ms.  128-thread tiles capped at 168 / 128 registers (3 / 4 CTAs per
 //   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
+#if Z4C_NG == 3
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
 using RhsTile2 = TileCfg<16, 4, 4, 3, 1>;
+#else
+// 4 ghosts: the halo tile grows to 24 x 12 x 10 (23 KB); to keep 2 CTAs per SM the P/Q tiles are read by batched
+// global loads instead of TMA (93 KB of shared memory per CTA)
+using RhsTile = TileCfg<16, 4, 2, 3, 2, false, false>;
+using RhsTile2 = TileCfg<16, 4, 4, 3, 1, false, false>;
+#endif
 // variant 4: P/Q by batched global loads + early parking. Measured 0.189 ms per launch at 64^3 against 0.183 ms for the
 // default; with the freed shared memory spent on a 5-deep ring instead it was 0.187 ms: neither the late tiles nor the
 // register pressure of the field stream is what limits the default kernel.
+#if Z4C_NG == 3
 using RhsTile5 = TileCfg<16, 4, 2, 3, 2, false>;
+#else
+using RhsTile5 = RhsTile;
+#endif
 
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, 2)
         int* L = lists + a * 3 * Cfg::MAXLIST;
         int cnt = 0;
         for (int l = c0[a]; l < c0[a] + T[a] && l < g.n; ++l) {
-          int tb[4], tl[4];
+          int tb[NG + 1], tl[NG + 1];
           const int nt = push_targets(l, bxyz[a], g.n, g.nb[a], g.bc, tb, tl);
           for (int q = 0; q < nt; ++q) {
             L[cnt] = l - c0[a]; L[Cfg::MAXLIST + cnt] = tb[q]; L[2 * Cfg::MAXLIST + cnt] = tl[q];
@@ -279,7 +279,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, 2)
   }
 }
 
+#if Z4C_NG == 3
 using StageTile = PersistCfg<16, 4, 2, 4>;
+#else
+using StageTile = PersistCfg<16, 4, 2, 3>;   // (1 CTA per SM at this halo size; experimental variant)
+#endif
 
 template <class Cfg, int STAGE>
 inline cudaError_t launch_stage_persistent_t(const CUtensorMap& map, const Pack& g, double* P, const FdConst& fd,

@@ -15,7 +15,8 @@ import numpy as np
 NF = 22
 Z4C_OK, Z4C_EINVAL, Z4C_ECUDA, Z4C_ESTATE = 0, -1, -2, -3
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libz4c.so")
+LIB_PATH = os.path.join(_HERE, "libz4c.so")            # built with 3 ghost zones (4th-order stencils)
+LIB_PATH_NG4 = os.path.join(_HERE, "libz4c_ng4.so")    # built with 4 ghost zones (6th-order stencils)
 
 # every symbol include/z4c.h declares
 SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_initial_data", "z4c_step",
@@ -48,15 +49,17 @@ def make_params(p) -> z4c_params:
     return o
 
 
-_lib = None
+_libs = {}
 
 
-def load_library(path: Optional[str] = None):
-    """dlopen libz4c.so and declare the prototypes. Raises if the library is not built."""
-    global _lib
-    if _lib is not None and path is None:
-        return _lib
-    path = path or LIB_PATH
+def load_library(path: Optional[str] = None, ng: int = 3):
+    """dlopen the library built for `ng` ghost zones and declare the prototypes. Raises if it is not built."""
+    if path is None and ng in _libs:
+        return _libs[ng]
+    if path is None and ng not in (3, 4):
+        raise ValueError("the library is built for ng = 3 (4th order) and ng = 4 (6th order)")
+    default = LIB_PATH if ng == 3 else LIB_PATH_NG4
+    path = path or default
     if not os.path.exists(path):
         raise RuntimeError(f"{path} is missing: build it with `python -m paper_2409_10383_b200.build` "
                            "(there is no CPU fallback)")
@@ -92,8 +95,8 @@ def load_library(path: Optional[str] = None):
                "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
                "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64"):
         getattr(L, fn).restype = C.c_int
-    if path == LIB_PATH:
-        _lib = L
+    if path == default:
+        _libs[ng] = L
     return L
 
 
@@ -111,7 +114,7 @@ class Z4c:
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the Z4c path has no CPU fallback")
         self.torch = torch
-        self.lib = load_library()
+        self.lib = load_library(ng=int(p.ng))
         self.p = p
         self.cp = make_params(p)
         self.device = torch.device(device)

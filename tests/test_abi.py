@@ -31,8 +31,10 @@ def header_symbols():
 def test_header_symbols_all_exported(lib):
     syms = header_symbols()
     assert sorted(Z.SYMBOLS) == syms
+    lib4 = Z.load_library(ng=4)            # the 4-ghost / 6th-order build exports the same ABI
     for s in syms:
         assert hasattr(lib, s), s
+        assert hasattr(lib4, s), s
 
 
 def test_library_is_sm100a_only():
@@ -47,6 +49,10 @@ def test_size_queries(lib):
     assert lib.z4c_state_bytes(C.byref(cp)) == 22 * 64 * 38 ** 3 * 8          # 618 MB
     wb = lib.z4c_workspace_bytes(C.byref(cp))
     assert wb >= 2 * 22 * 64 * 32 ** 3 * 8 and wb % 256 == 0
+    cp4 = Z.make_params(p)
+    cp4.ng = 4
+    assert lib.z4c_state_bytes(C.byref(cp4)) == 0                       # each build accepts only its own ghost count
+    assert Z.load_library(ng=4).z4c_state_bytes(C.byref(cp4)) == 22 * 64 * 40 ** 3 * 8
     bad = Z.make_params(p)
     bad.ng = 2
     assert lib.z4c_state_bytes(C.byref(bad)) == 0 and lib.z4c_workspace_bytes(C.byref(bad)) == 0

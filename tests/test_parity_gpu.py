@@ -43,6 +43,10 @@ CASES = {
     "smooth_periodic": lambda: (I.params_noise(12, (2, 1, 2), dx=0.05), "smooth"),
     "smooth_outflow": lambda: (replace(I.params_noise(16, (1, 2, 2), dx=0.05), bc=1, shift_eta=1.0), "smooth"),
     "smooth_n32": lambda: (I.params_noise(32, (1, 1, 1), dx=0.03), "smooth"),
+    # NEXT-1: 4 ghost zones, 6th-order stencils (libz4c_ng4.so)
+    "o6_noise_ragged": lambda: (replace(I.params_noise(10, (2, 1, 2)), ng=4), "noise"),
+    "o6_smooth_periodic": lambda: (replace(I.params_noise(16, (2, 1, 1), dx=0.05), ng=4), "smooth"),
+    "o6_smooth_outflow": lambda: (replace(I.params_noise(12, (1, 2, 2), dx=0.05), ng=4, bc=1, shift_eta=1.0), "smooth"),
 }
 
 
@@ -225,7 +229,7 @@ def test_puncture_small_20_steps(Z, oracle):
 
 
 # ------------------------------------------------------------------------------ S5
-@pytest.mark.parametrize("name", ["smooth_periodic", "smooth_outflow", "noise_ragged"])
+@pytest.mark.parametrize("name", ["smooth_periodic", "smooth_outflow", "noise_ragged", "o6_smooth_outflow"])
 def test_constraints_parity(Z, oracle, name):
     p, u = case_data(name)
     sim = make(Z, p, u)
