@@ -28,6 +28,7 @@ from paper_2409_10383_b200 import inputs as I  # noqa: E402
 # Algorithmic work per cell (flop census = oracle/z4c_oracle.cpp oz4c_count_flops,
 # add = mul = div = 1, no FMA fusion assumed; checked by tests/test_oracle_pins.py::test_flop_census).
 RHS_FLOPS_PER_CELL = 6034
+RHS_FLOPS_PER_CELL_O6 = 8059      # same census with the 6th-order stencil set (ng = 4)
 # doubles moved per cell and RK4 step by the O6 recurrence: 616, plus the ghost fill
 STEP_DOUBLES_PER_CELL = 616
 GHOST_DOUBLES_PER_GHOST_CELL_STEP = 4 * 22 * 2
@@ -40,7 +41,11 @@ WORKLOAD_LABELS = {
     "linear_wave_64": "configs[1]: linear wave 64^3 = 64 blocks of 16^3 (+3 ghosts), periodic",
     "puncture_128": "configs[2]: single puncture 128^3 = 64 blocks of 32^3, outflow-copy",
     "bbh_256": "configs[3]: two punctures 256^3 = 512 blocks of 32^3, outflow-copy",
+    "linear_wave_o6_256": "NEXT-1 / paper Table 1 shape: linear wave 256^3 = 64 blocks of 64^3 (+4 ghosts), 6th order",
 }
+# the paper's own figure for the Table 1 workload (A100, 64^3 blocks, VRAM filled, 6th order + RK4):
+# another machine, context only
+PAPER_A100_ZCPS = 1.36e7
 
 
 def workload(name: str):
@@ -54,6 +59,9 @@ def workload(name: str):
     if name == "bbh_256":
         p, u, _ = I.config(3)
         return p, u, "configs[3]: two punctures 256^3 = 512 blocks of 32^3, outflow-copy"
+    if name == "linear_wave_o6_256":
+        p = replace(I.params_linear_wave(256, 64), ng=4)
+        return p, I.linear_wave_data(p), WORKLOAD_LABELS[name]
     if name.startswith("noise_"):            # configs[4] load sweep: noise_<n>_<nbx>x<nby>x<nbz>
         _, n, lat = name.split("_")
         nb = tuple(int(v) for v in lat.split("x"))
@@ -161,6 +169,9 @@ def oracle_sample(name: str):
         p = I.params_linear_wave(64, 16)
         ps = replace(p, nb=(4, 1, 1))   # 64 x 16 x 16 periodic slab of the same wave
         return ps, I.linear_wave_data(ps), "64x16x16 periodic slab of the 64^3 wave (same per-cell arithmetic)"
+    if name == "linear_wave_o6_256":
+        ps = replace(I.params_linear_wave(256, 16), nb=(16, 1, 1), ng=4)
+        return ps, I.linear_wave_data(ps), "256x16x16 periodic slab of the 256^3 wave, 6th-order stencils"
     if name in ("puncture_128", "bbh_256"):
         p, u, _ = I.config(2 if name == "puncture_128" else 3)
         lo = p.N[0] // 2 - 16
@@ -267,7 +278,8 @@ def run_ours(args):
     rhs_ms = kt["rhs"] / (4 * K)
     fp64_peak = sim.probe_fp64()
     hbm_peak, hbm_src = measured_peaks()
-    rhs_tflops = RHS_FLOPS_PER_CELL * ncells / (rhs_ms * 1e-3) * 1e-12
+    flops_cell = RHS_FLOPS_PER_CELL if p.ng == 3 else RHS_FLOPS_PER_CELL_O6
+    rhs_tflops = flops_cell * ncells / (rhs_ms * 1e-3) * 1e-12
     rhs_gbs = RHS_DOUBLES_PER_CELL * 8 * ncells / (rhs_ms * 1e-3) * 1e-9
     g = p.ng
     ghost_cells = p.nblocks * ((p.n + 2 * g) ** 3 - p.n ** 3)
@@ -301,7 +313,8 @@ def run_ours(args):
         line = {
             "metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": zcps, "unit": "zone-cycles/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": (zcps / PAPER_A100_ZCPS) if args.workload == "linear_wave_o6_256" and world == 1 else None,
+            "dtype": "f64", "data": "synthetic",
             "config": {"workload": label, "cells_per_gpu": ncells, "blocks": p.nblocks, "n": p.n, "ghosts": g,
                        "parallelism": "replicas" if world > 1 else "1 GPU",
                        "l2": "no flush: y+P+Q working set %.0f MB > 126 MB L2" %
@@ -316,7 +329,7 @@ def run_ours(args):
                          "unit": "TFLOP/s", "frac": rhs_tflops / fp64_peak,
                          "traffic": profiled_traffic(args.workload),
                          "peak_source": "measured live: z4c_probe_fp64 DFMA loop (nominal %.1f at 1965 MHz)" % FP64_NOMINAL_TFLOPS,
-                         "flops_per_cell": RHS_FLOPS_PER_CELL, "ms_per_launch": rhs_ms,
+                         "flops_per_cell": flops_cell, "ms_per_launch": rhs_ms,
                          "hbm_gbs_algorithmic": rhs_gbs, "share_of_step": kt["rhs"] / total_kt},
             "step_roofline": {"bound": "hbm", "achieved": step_bytes * K / (ms_local * 1e-3) * 1e-9, "peak": hbm_peak,
                               "unit": "GB/s", "frac": step_bytes * K / (ms_local * 1e-3) * 1e-9 / hbm_peak,

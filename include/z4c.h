@@ -57,7 +57,8 @@ typedef struct z4c_ctx z4c_ctx; /* opaque, host memory, owned by the library */
 
 typedef struct {
   int32_t n;      /* interior cells per MeshBlock edge (16, 32, 64 are the tuned sizes; any n >= 6 accepted) */
-  int32_t ng;     /* ghost zones per side; must be 3 (4th order by the rule at PAPER.md:124) */
+  int32_t ng;     /* ghost zones per side = stencil half-width, fixed per build: 3 in libz4c.so (4th order by the rule
+                     at PAPER.md:124), 4 in libz4c_ng4.so (6th order); other values: Z4C_EINVAL */
   int32_t nb[3];  /* block lattice (x,y,z); N_b = nb[0]*nb[1]*nb[2] */
   int32_t bc;     /* 0 periodic; 1 outflow-copy: ghost = nearest interior cell, all six faces */
   double xmin[3]; /* lower corner of the domain */

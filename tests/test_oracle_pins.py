@@ -420,6 +420,9 @@ def test_flop_census(oracle):
     c2 = oracle.count_flops(p, u, 3, 4, 5)["rhs"]
     tot2 = c2["add"] + c2["mul"] + c2["div"]
     assert bench.RHS_FLOPS_PER_CELL <= tot2 <= bench.RHS_FLOPS_PER_CELL + 66 and c2["add"] == c["add"]
+    p6 = replace(I.params_noise(10, (1, 1, 1)), ng=4)
+    c6 = oracle.count_flops(p6, I.minkowski(p6), 5, 5, 5)["rhs"]
+    assert c6["add"] + c6["mul"] + c6["div"] == bench.RHS_FLOPS_PER_CELL_O6
 
 
 # ---------------------------------------------------------------- NEXT-1: 6th-order stencil set (4 ghosts)
