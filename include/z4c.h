@@ -104,6 +104,14 @@ int z4c_step(z4c_ctx* ctx, int nsteps);
  * Returns Z4C_ESTATE if the device error flag is set. */
 int z4c_constraints(z4c_ctx* ctx, double* out, double* d_percell);
 
+/* AMR refinement indicators per MeshBlock (sections 3.3.1-3.3.2; no regridding here): for every
+ * block b, d_minchi[b] = min of chi and d_maxdchi[b] = max of |grad chi| (Euclidean norm of the scheme's centred first
+ * derivative) over the block's interior cells, d_flags[b] = (min chi < chi_min ? 1 : 0) | (max |grad chi| > dchi_max ?
+ * 2 : 0), i.e. bit 0 = the chi-min criterion, bit 1 = the d-chi-max criterion. All three outputs are device pointers
+ * to N_b elements, each may be NULL (not all). Ghosts must be valid. Async. */
+int z4c_refine_indicators(z4c_ctx* ctx, double chi_min, double dchi_max, double* d_minchi, double* d_maxdchi,
+                          int32_t* d_flags);
+
 /* Inverse of z4c_set_initial_data: gather the interior cells of the pack into an interior
  * array. host pointer (on_device = 0; synchronises; staged through the workspace, so the RK
  * registers must not be live, i.e. not between stages -- always true between API calls) or

@@ -61,6 +61,7 @@ def lib():
         L.oz4c_num_intermediates.restype = C.c_int
         L.oz4c_intermediates.argtypes = [pp, dp, dp]
         L.oz4c_count_flops.argtypes = [pp, dp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
+        L.oz4c_refine_indicators.argtypes = [pp, dp, C.c_int, dp, dp]
         L.oz4c_num_threads.restype = C.c_int
         L.oz4c_set_num_threads.argtypes = [C.c_int]
         _lib = L
@@ -152,6 +153,16 @@ def intermediates(p, u: np.ndarray) -> np.ndarray:
     out = np.empty((nq,) + u.shape[1:])
     lib().oz4c_intermediates(C.byref(_op(p, _N_of(u))), _ptr(u), _ptr(out))
     return out
+
+
+def refine_indicators(p, u: np.ndarray, n: int):
+    """NEXT-4: per-block (min chi, max |grad chi|), blocks of n^3 cells in lattice order."""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    N = _N_of(u)
+    nb = (N[0] // n) * (N[1] // n) * (N[2] // n)
+    mn, mx = np.empty(nb), np.empty(nb)
+    lib().oz4c_refine_indicators(C.byref(_op(p, N)), _ptr(u), int(n), _ptr(mn), _ptr(mx))
+    return mn, mx
 
 
 def count_flops(p, u: np.ndarray, i: int, j: int, k: int):

@@ -305,6 +305,42 @@ void oz4c_constraints(const Params* P, const double* u, double* out, double* per
   out[4] = std::sqrt(sT / nc); out[5] = mT; out[6] = std::sqrt(sZ / nc); out[7] = mZ;
 }
 
+// NEXT-4 (sections 3.3.1-3.3.2): per-MeshBlock refinement indicators. Blocks of n^3 cells tile
+// the global array (block id = (bz*nby + by)*nbx + bx). minchi[b] = min over the block of chi (chi-min criterion:
+// refine if it falls below a threshold); maxdchi[b] = max over the block of |grad chi| (d-chi-max criterion: refine if it
+// exceeds a threshold), with grad = the scheme's centred first derivative and |.| the Euclidean norm (reading Q20).
+void oz4c_refine_indicators(const Params* P, const double* u, int n, double* minchi, double* maxdchi) {
+  View V(*P, u);
+  const int nbx = P->N[0] / n, nby = P->N[1] / n, nbz = P->N[2] / n;
+  const bool o6 = sixth_order(*P);
+  for (int bz = 0; bz < nbz; ++bz)
+    for (int by = 0; by < nby; ++by)
+      for (int bx = 0; bx < nbx; ++bx) {
+        double mn = INFINITY, mx = 0.0;
+        for (int k = bz * n; k < (bz + 1) * n; ++k)
+          for (int j = by * n; j < (by + 1) * n; ++j)
+            for (int i = bx * n; i < (bx + 1) * n; ++i) {
+              const int c[3] = {i, j, k};
+              double g2 = 0.0;
+              for (int a = 0; a < 3; ++a) {
+                double l[9];
+                for (int s = -4; s <= 4; ++s) {
+                  int q[3] = {c[0], c[1], c[2]};
+                  q[a] += s;
+                  l[s + 4] = V.at(CHI, q[0], q[1], q[2]);
+                }
+                const double d = o6 ? d1_centred6(&l[4], P->dx) : d1_centred(&l[4], P->dx);
+                g2 += d * d;
+              }
+              mn = std::fmin(mn, V.at(CHI, i, j, k));
+              mx = std::fmax(mx, std::sqrt(g2));
+            }
+        const int b = (bz * nby + by) * nbx + bx;
+        minchi[b] = mn;
+        maxdchi[b] = mx;
+      }
+}
+
 // Pins P2: apply one stencil of O3 to a single scalar array f[Nz][Ny][Nx].
 // kind: 0 centred-1st(axis a), 1 centred-2nd(axis a), 2 mixed(a,b), 3 upwind+ (a), 4 upwind- (a),
 //       5 KO summed over the three axes including the eps/(64h) factor

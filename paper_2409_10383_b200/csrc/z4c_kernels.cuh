@@ -369,6 +369,41 @@ __global__ void __launch_bounds__(K4_THREADS)
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-4: per-MeshBlock refinement indicators: min chi and max |grad chi| over the interior
+// cells of each block, and the two flags (bit 0: min chi < chi_min, bit 1: max |grad chi| > dchi_max). One CTA per
+// block; min/max reductions are exact in any order, so the result is deterministic.
+// ---------------------------------------------------------------------------------------------
+constexpr int KR_THREADS = 256;
+__global__ void __launch_bounds__(KR_THREADS)
+    k_refine_indicators(Pack g, const double* __restrict__ y, FdConst fd, double chi_min, double dchi_max,
+                        double* __restrict__ minchi, double* __restrict__ maxdchi, int* __restrict__ flags) {
+  __shared__ double smn[KR_THREADS / 32], smx[KR_THREADS / 32];
+  const int b = blockIdx.x;
+  const double* chi = y + (long long)CHI * g.fs + (long long)b * g.m3;
+  double mn = INFINITY, mx = 0.0;
+  for (int r = threadIdx.x; r < g.n3; r += KR_THREADS) {
+    const int i = r % g.n, j = (r / g.n) % g.n, k = r / (g.n * g.n);
+    const double* p = chi + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
+    const double dx = d1_raw(p, 1) * fd.inv12h, dy = d1_raw(p, g.m) * fd.inv12h, dz = d1_raw(p, g.m2) * fd.inv12h;
+    mn = fmin(mn, __ldg(p));
+    mx = fmax(mx, sqrt(dx * dx + dy * dy + dz * dz));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    mn = fmin(mn, __shfl_down_sync(0xffffffffu, mn, o));
+    mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+  }
+  if ((threadIdx.x & 31) == 0) { smn[threadIdx.x >> 5] = mn; smx[threadIdx.x >> 5] = mx; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < KR_THREADS / 32; ++w) { mn = fmin(mn, smn[w]); mx = fmax(mx, smx[w]); }
+    if (minchi) minchi[b] = mn;
+    if (maxdchi) maxdchi[b] = mx;
+    if (flags) flags[b] = (mn < chi_min ? 1 : 0) | (mx > dchi_max ? 2 : 0);
+  }
+}
+
 // second pass: one CTA, fixed order. out[8] = {H_rms,H_max,M_rms,M_max,Theta_rms,Theta_max,Z_rms,Z_max}
 __global__ void __launch_bounds__(K4_THREADS)
     k_constraints_final(const double* __restrict__ partial, int nparts, double ncell, double* __restrict__ out) {

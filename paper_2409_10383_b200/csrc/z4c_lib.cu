@@ -442,6 +442,14 @@ int z4c_constraints(z4c_ctx* c, double* out, double* d_percell) {
   return read_flag(c);
 }
 
+int z4c_refine_indicators(z4c_ctx* c, double chi_min, double dchi_max, double* d_minchi, double* d_maxdchi,
+                          int32_t* d_flags) {
+  if (!c || (!d_minchi && !d_maxdchi && !d_flags)) return Z4C_EINVAL;
+  k_refine_indicators<<<c->g.nblk, KR_THREADS, 0, c->stream>>>(c->g, c->y, c->fd, chi_min, dchi_max, d_minchi,
+                                                                d_maxdchi, (int*)d_flags);
+  return check_launch(c, "k_refine_indicators");
+}
+
 int z4c_get_interior(z4c_ctx* c, double* interior, int on_device) {
   if (!c || !interior) return Z4C_EINVAL;
   const size_t bytes = (size_t)NF * (size_t)c->g.ncell * sizeof(double);

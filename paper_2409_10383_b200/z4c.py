@@ -20,7 +20,7 @@ LIB_PATH_NG4 = os.path.join(_HERE, "libz4c_ng4.so")    # built with 4 ghost zone
 
 # every symbol include/z4c.h declares
 SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_initial_data", "z4c_step",
-           "z4c_constraints", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
+           "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
            "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
            "z4c_probe_fp64", "z4c_time",
            "z4c_last_error", "z4c_destroy"]
@@ -73,6 +73,7 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_set_initial_data.argtypes = [vp, dp, C.c_int]
     L.z4c_step.argtypes = [vp, C.c_int]
     L.z4c_constraints.argtypes = [vp, C.POINTER(C.c_double), dp]
+    L.z4c_refine_indicators.argtypes = [vp, C.c_double, C.c_double, dp, dp, dp]
     L.z4c_get_interior.argtypes = [vp, dp, C.c_int]
     L.z4c_fill_ghosts.argtypes = [vp]
     L.z4c_eval_rhs.argtypes = [vp, dp]
@@ -91,7 +92,7 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_last_error.restype = C.c_char_p
     L.z4c_destroy.argtypes = [vp]
     L.z4c_destroy.restype = None
-    for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_get_interior",
+    for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior",
                "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
                "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64"):
         getattr(L, fn).restype = C.c_int
@@ -178,6 +179,19 @@ class Z4c:
             self._check(self.lib.z4c_constraints(self.h, out, pc.data_ptr() if percell else None))
         res = np.array(list(out))
         return (res, pc.cpu().numpy()) if percell else res
+
+    def refine_indicators(self, chi_min: float, dchi_max: float):
+        """z4c_refine_indicators: (min chi, max |grad chi|, flags) per block as numpy arrays."""
+        torch = self.torch
+        nblk = self.p.nb[0] * self.p.nb[1] * self.p.nb[2]
+        with torch.cuda.device(self.device):
+            mn = torch.empty(nblk, dtype=torch.float64, device=self.device)
+            mx = torch.empty(nblk, dtype=torch.float64, device=self.device)
+            fl = torch.empty(nblk, dtype=torch.int32, device=self.device)
+            self._check(self.lib.z4c_refine_indicators(self.h, float(chi_min), float(dchi_max), mn.data_ptr(),
+                                                       mx.data_ptr(), fl.data_ptr()))
+            self._check(self.lib.z4c_sync(self.h))
+        return mn.cpu().numpy(), mx.cpu().numpy(), fl.cpu().numpy()
 
     def get_interior(self, out=None) -> np.ndarray:
         """Host copy of the interior cells (numpy). If `out` is a CUDA tensor, fills it on the device instead."""

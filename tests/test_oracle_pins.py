@@ -511,3 +511,45 @@ def test_N1_sixth_order_convergence_and_minkowski(oracle):
         exact = I.linear_wave_data(pp, t=16 * pp.dt)
         e[name] = np.abs(out[I.GYY] - exact[I.GYY]).max()
     assert e["o6"] < e["o4"] / 5.0, e
+
+
+# ---------------------------------------------------------------- NEXT-4: chi-min / d-chi-max refinement indicators
+def test_N4_refinement_indicators(oracle):
+    """PAPER.md:132-142. min chi per block against numpy's own block minimum; |grad chi| against the closed form for
+    Brill-Lindquist data; and the paper's qualitative statement: in an unequal-mass binary the
+    smaller hole has the larger gradient of chi, so d-chi-max refines it more."""
+    p = I.params_puncture(48, 12, 3.0, 2.0)                    # 4^3 blocks of 12^3, dx = 0.125
+    m1, m2 = 0.75, 0.25
+    pos = ((-1.3, 0.4, 0.3), (1.4, -0.5, 0.2))                 # both inside a block, off the cell centres
+    u = I.puncture_data(p, (m1, m2), pos)
+    mn, mx = oracle.refine_indicators(p, u, p.n)
+    n, nb = p.n, p.nb[0]
+    blocks = u[I.CHI].reshape(nb, n, nb, n, nb, n).transpose(0, 2, 4, 1, 3, 5).reshape(nb ** 3, -1)
+    assert np.array_equal(mn, blocks.min(axis=1))
+    # closed form: chi = psi^-4, grad chi = -4 psi^-5 grad psi, grad psi = -sum m_i (x - x_i) / (2 r_i^3)
+    z, y, x = I.cell_centres(p)
+    psi = 1.0
+    gp = [0.0, 0.0, 0.0]
+    rmin = np.inf
+    for m, c in zip((m1, m2), pos):
+        d = [x - c[0], y - c[1], z - c[2]]
+        r = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
+        rmin = np.minimum(rmin, r / m)
+        psi = psi + m / (2 * r)
+        for a in range(3):
+            gp[a] = gp[a] - m * d[a] / (2 * r ** 3)
+    gnorm = 4 * psi ** -5 * np.sqrt(gp[0] ** 2 + gp[1] ** 2 + gp[2] ** 2)
+    per_block = lambda a: a.reshape(nb, n, nb, n, nb, n).transpose(0, 2, 4, 1, 3, 5).reshape(nb ** 3, -1)  # noqa: E731
+    exact = per_block(gnorm).max(axis=1)
+    far = np.nonzero(per_block(rmin).min(axis=1) > 4.0)[0]     # blocks at least 4 m_i away from puncture i: smooth data
+    assert len(far) >= 10 and np.abs(mx[far] / exact[far] - 1).max() < 1e-3     # 4th-order truncation
+    # block of each puncture (lattice order: b = (bz*nb + by)*nb + bx)
+    def block_of(c):
+        i = [int((c[a] - p.xmin[a]) / p.dx) // n for a in range(3)]
+        return (i[2] * nb + i[1]) * nb + i[0]
+    big, small = block_of(pos[0]), block_of(pos[1])
+    # single-puncture closed form: max |grad chi| = 8 x^2 / (m (1+x)^5) at x = m/2r = 2/3, i.e. 0.2765/m -- it grows
+    # as the mass falls, which is why d-chi-max gives the smaller hole more levels (PAPER.md:138, 142)
+    assert mx[small] > 2.0 * mx[big]
+    assert 0.5 * 0.2765 / m1 < mx[big] < 1.5 * 0.2765 / m1
+    assert mn[big] < 0.3 and mn[small] < 0.3             # chi-min (threshold 0.3, PAPER.md:207) flags both

@@ -254,3 +254,18 @@ def test_run_to_run_determinism(Z):
         outs.append(sim.state.cpu().numpy())
         sim.close()
     assert np.array_equal(outs[0], outs[1])
+
+
+# ------------------------------------------------------------------------------ NEXT-4 refinement indicators
+@pytest.mark.parametrize("ng", [3, 4])
+def test_refinement_indicators_parity(Z, oracle, ng):
+    p = replace(I.params_puncture(48, 12, 3.0, 2.0), ng=ng)
+    u = I.puncture_data(p, (0.75, 0.25), ((-1.3, 0.4, 0.3), (1.4, -0.5, 0.2)))
+    sim = make(Z, p, u)
+    mn, mx, fl = sim.refine_indicators(0.3, 0.5)
+    rmn, rmx = oracle.refine_indicators(p, oracle.enforce(p, u)[0], p.n)
+    assert np.array_equal(mn, rmn)                                   # a minimum of stored values: bit-exact
+    assert np.abs(mx / rmx - 1).max() <= 1e-13
+    ref_flags = (rmn < 0.3).astype(np.int32) | ((rmx > 0.5).astype(np.int32) << 1)
+    assert np.array_equal(fl, ref_flags) and fl.max() == 3 and fl.min() == 0
+    sim.close()
