@@ -138,3 +138,59 @@ def test_config5_periodic_tiling_invariance(Z, oracle, n, nb):
         assert err.max() <= 1e-10, dict(zip(I.FIELD_NAMES, err))
     big.close()
     small.close()
+
+
+def test_64bit_indexing_pack_larger_than_2_31_elements(Z):
+    """288 blocks of 64^3: the state alone is 22 x 288 x 70^3 = 2.17e9 doubles (> 2^31), ~100 GB on the device in total.
+    Periodic-tiling invariance against the 8-block pack, compared on the device."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs ~100 GB of free device memory")
+    tile = (2, 2, 2)
+    p = I.params_noise(64, (8, 6, 6), 0.1)
+    ps = replace(p, nb=tile)
+    assert 22 * p.nblocks * 70 ** 3 > 2 ** 31
+    base = torch.from_numpy(I.noise_data(ps, 1000)).cuda()
+    small = Z.Z4c(ps)
+    small.set_initial_data(base)
+    small.step(3)
+    small.sync()
+    ref = torch.empty_like(base)
+    small.get_interior(ref)
+    small.close()
+    reps = (1, p.nb[2] // 2, p.nb[1] // 2, p.nb[0] // 2)
+    u = base.repeat(*reps).contiguous()
+    big = Z.Z4c(p)
+    big.use_graph(True)
+    big.set_initial_data(u)
+    big.step(3)
+    big.sync()
+    big.get_interior(u)                       # reuse the buffer for the result
+    ok = True
+    for kz in range(reps[1]):                 # tile by tile: no second 13 GB array
+        for ky in range(reps[2]):
+            for kx in range(reps[3]):
+                ok &= bool(torch.equal(u[:, kz * 128:(kz + 1) * 128, ky * 128:(ky + 1) * 128, kx * 128:(kx + 1) * 128], ref))
+    assert ok
+    big.close()
+    del u, base, ref
+    torch.cuda.empty_cache()
+
+
+def test_zero_steps_and_reinitialisation(Z):
+    p = I.params_noise(16, (1, 1, 2))
+    u = I.noise_data(p, 7)
+    sim = Z.Z4c(p)
+    sim.set_initial_data(u)
+    before = sim.state.clone()
+    sim.step(0)                                # no-op
+    sim.sync()
+    assert bool((sim.state == before).all()) and sim.time() == 0.0
+    sim.step(2)
+    sim.set_initial_data(u)                    # resets time and the RK registers
+    sim.sync()
+    assert bool((sim.state == before).all()) and sim.time() == 0.0
+    with pytest.raises(Z.Z4cError):
+        sim.step(-1)
+    sim.close()
