@@ -162,12 +162,10 @@ __device__ __forceinline__ void ricci_conformal(const double* g, const double* g
         r += 0.5 * Gd[k] * (Gl[i][sym(j, k)] + Gl[j][sym(i, k)]);
 #pragma unroll
         for (int m = 0; m < 3; ++m) {
-          // gi^{lm}( Gu^k_{li} Gl_{jkm} + Gu^k_{lj} Gl_{ikm} + Gu^k_{im} Gl_{klj} )
-          r += T[k][m][i] * Gl[j][sym(k, m)] + T[k][m][j] * Gl[i][sym(k, m)];
-          // third term: Gu^k_{im} gi^{lm} Gl_{k l j} = Gu^k_{im} * (raise 2nd index of Gl_k..) ;
-          // gi^{lm} Gl_{klj} = g_{kq} T[q][m][j]
-          r += Gu[k][sym(i, m)] *
-               (g[sym(k, 0)] * T[0][m][j] + g[sym(k, 1)] * T[1][m][j] + g[sym(k, 2)] * T[2][m][j]);
+          // gi^{lm}( Gu^k_{li} Gl_{jkm} + Gu^k_{lj} Gl_{ikm} + Gu^k_{im} Gl_{klj} ) with T[k][m][.] = gi^{lm} Gu^k_{l .};
+          // third term: gi^{lm} Gu^q_{im} Gl_{qlj} = gi^{lm} Gl_{q im} Gu^q_{lj} = Gl_{k im} T[k][m][j]  (lower q on the
+          // first factor instead of the second: 3 FMAs per (k, m) instead of 6)
+          r += T[k][m][i] * Gl[j][sym(k, m)] + T[k][m][j] * Gl[i][sym(k, m)] + T[k][m][j] * Gl[k][sym(i, m)];
         }
       }
       Rt[p] = r;
