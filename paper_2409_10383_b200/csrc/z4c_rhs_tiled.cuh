@@ -85,7 +85,7 @@ __host__ __device__ constexpr int stream_field(int it) { return it < 3 ? BETAX +
 // One axis of one field out of the shared-memory tile. t points at the cell, S is the compile-time stride.
 template <int S, bool WANT_D1, bool WANT_D2>
 __device__ __forceinline__ void axis_tile(const double* t, const double c, const double bw, const double aw,
-                                          const FdConst& fd, double& d1, double& d2, double& adv, double& ko) {
+                                          const FdConst& fd, double& d1, double& d2, double& adv) {
 #if Z4C_NG == 3
   const double lm3 = t[-3 * S], lm2 = t[-2 * S], lm1 = t[-S], lp1 = t[S], lp2 = t[2 * S], lp3 = t[3 * S];
   const double e1 = lp1 - lm1, e2 = lp2 - lm2, e3 = lp3 - lm3;
@@ -107,8 +107,8 @@ __device__ __forceinline__ void axis_tile(const double* t, const double c, const
   const double k = 56.0 * s1 - 28.0 * s2 + 8.0 * s3 - s4;
   const double sy = 104.0 * e1 - 32.0 * e2 + 8.0 * e3 - e4;
 #endif
+  // bw = c_adv beta/(24h) [120h], aw = c_adv |beta|/(24h) + eps/(64h) [.., 256h]: advection and dissipation in two FMAs
   adv += bw * sy + aw * k;
-  ko += k;
 }
 
 // mixed second derivative from the tile, compile-time strides
@@ -133,10 +133,24 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
   constexpr bool W1 = need_d1(F), W2 = need_d2(F);
   const double c = t[0];
   u[F] = c;
-  double adv = 0.0, ko = 0.0, d1x = 0, d1y = 0, d1z = 0, d2x = 0, d2y = 0, d2z = 0;
-  axis_tile<1, W1, W2>(t, c, bw[0], aw[0], fd, d1x, d2x, adv, ko);
-  axis_tile<Cfg::SY, W1, W2>(t, c, bw[1], aw[1], fd, d1y, d2y, adv, ko);
-  axis_tile<Cfg::SZ, W1, W2>(t, c, bw[2], aw[2], fd, d1z, d2z, adv, ko);
+  double adv = 0.0, d1x = 0, d1y = 0, d1z = 0, d2x = 0, d2y = 0, d2z = 0;
+  // bw[a] = beta^a/(24h), aw[a] = |beta^a|/(24h) + eps/(64h) (the Kreiss-Oliger weight folded in) for fields whose
+  // advection is not switched by a gauge parameter; alpha and beta^i rebuild their weights with c_adv
+  double w1[3], w2[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (F == ALPHA || F >= BETAX) {
+      const double cadv = (F == ALPHA) ? sp.lapse_advect : sp.shift_advect;
+      w1[a] = cadv * bw[a];
+      w2[a] = cadv * (aw[a] - fd.ko) + fd.ko;
+    } else {
+      w1[a] = bw[a];
+      w2[a] = aw[a];
+    }
+  }
+  axis_tile<1, W1, W2>(t, c, w1[0], w2[0], fd, d1x, d2x, adv);
+  axis_tile<Cfg::SY, W1, W2>(t, c, w1[1], w2[1], fd, d1y, d2y, adv);
+  axis_tile<Cfg::SZ, W1, W2>(t, c, w1[2], w2[2], fd, d1z, d2z, adv);
   if (W1) { D.d1[F][0] = d1x; D.d1[F][1] = d1y; D.d1[F][2] = d1z; }
   if (W2) {
     double d2[6];
@@ -146,9 +160,8 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
     d2[sym(1, 2)] = mixed_tile<Cfg::SY, Cfg::SZ>(t) * fd.inv144h2;
     consume_d2<F>(d2, D);
   }
-  const double cadv = (F == ALPHA) ? sp.lapse_advect : (F >= BETAX ? sp.shift_advect : 1.0);
   // parked in shared memory until the sources are assembled: 22 doubles fewer live through the tensor algebra
-  out[F * Cfg::THREADS] = cadv * adv + ko * fd.ko;
+  out[F * Cfg::THREADS] = adv;
   if (Cfg::EARLY_PARK) park_field_early<F>(D, out + (Cfg::E_OFF - Cfg::S_OFF) / 8, Cfg::THREADS);
 }
 
@@ -282,7 +295,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     mbar_wait(&full[a], 0);
     const double beta = reinterpret_cast<const double*>(tiles + a * Cfg::STAGE_BYTES)[toff];
     bw[a] = beta * (0.5 * fd.inv12h);
-    aw[a] = fabs(beta) * (0.5 * fd.inv12h);
+    aw[a] = fabs(beta) * (0.5 * fd.inv12h) + fd.ko;
   }
   double u[NF];
   double* park = reinterpret_cast<double*>(tiles + Cfg::S_OFF) + tid;

@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, 2)
       mbar_wait(&full[n % Cfg::NSTAGE], (n / Cfg::NSTAGE) & 1);
       const double beta = reinterpret_cast<const double*>(ring + (n % Cfg::NSTAGE) * Cfg::STAGE_BYTES)[toff];
       bw[a] = beta * (0.5 * fd.inv12h);
-      aw[a] = fabs(beta) * (0.5 * fd.inv12h);
+      aw[a] = fabs(beta) * (0.5 * fd.inv12h) + fd.ko;
     }
     double* park = sA + tid;
     PersistLoop<Cfg, 0>::run(&map, ring, full, n0, toff, cur, nxt, has_next, active, bw, aw, fd, sp, u, D, park);
