@@ -422,6 +422,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   64^3 wave: 0.202 ms per launch against 0.213 ms for the 16x4x4 tile (256 threads, 1 CTA per SM);
 //   256^3 two punctures: 9.94 against 10.76 ms.  128-thread tiles capped at 168 / 128 registers (3 / 4 CTAs per
 //   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
+//   8-wide tiles (8x4x4, 8x8x2: 20 % fewer halo bytes) are 20 % slower: 64-byte rows halve the coalescing of the
+//   register / state rows and put two tile rows of a warp on the same shared-memory banks.
 #if Z4C_NG == 3
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
 using RhsTile2 = TileCfg<16, 4, 4, 3, 1>;
