@@ -553,3 +553,24 @@ def test_N4_refinement_indicators(oracle):
     assert mx[small] > 2.0 * mx[big]
     assert 0.5 * 0.2765 / m1 < mx[big] < 1.5 * 0.2765 / m1
     assert mn[big] < 0.3 and mn[small] < 0.3             # chi-min (threshold 0.3) flags both
+
+
+# ---------------------------------------------------------------- reading R-U1 (select-free upwinding on the GPU)
+@pytest.mark.parametrize("ng", [3, 4])
+def test_RU1_upwind_pair_identity(oracle, ng):
+    """DESIGN.md R-U1: D+ - D- of the one-sided pair is the Kreiss-Oliger bracket / (12h) [60h] and D+ + D- is an
+    antisymmetric centred stencil, so beta D^{sign beta} = [beta (D+ + D-) + |beta| (D+ - D-)]/2 needs no select.
+    Checked on the oracle's own one-sided stencils with random data varying along one axis."""
+    p = replace(I.params_noise(16, (1, 1, 1), 0.1), ng=ng, ko_eps=0.5)
+    rng = np.random.default_rng(3)
+    line = rng.uniform(-1, 1, 16)
+    f = np.broadcast_to(line[None, None, :], (16, 16, 16)).copy()
+    h = p.dx
+    dplus, dminus = oracle.stencil(p, f, 3, 0), oracle.stencil(p, f, 4, 0)
+    ko = oracle.stencil(p, f, 5)                       # only the x axis contributes for this data
+    c1, cko = (12.0, 64.0) if ng == 3 else (60.0, 256.0)
+    assert np.abs((dplus - dminus) - ko * (cko * h / p.ko_eps) / (c1 * h)).max() <= 1e-12 * np.abs(dplus).max()
+    # the symmetric part, written out: (e3 - 6 e2 + 21 e1)/(12h)  [(104 e1 - 32 e2 + 8 e3 - e4)/(60h)]
+    e = lambda s: np.roll(line, -s) - np.roll(line, s)     # noqa: E731  (periodic)
+    sym = (e(3) - 6 * e(2) + 21 * e(1)) / (12 * h) if ng == 3 else (104 * e(1) - 32 * e(2) + 8 * e(3) - e(4)) / (60 * h)
+    assert np.abs((dplus + dminus)[0, 0] - sym).max() <= 1e-12 * np.abs(dplus).max()
