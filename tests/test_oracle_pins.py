@@ -574,3 +574,157 @@ def test_RU1_upwind_pair_identity(oracle, ng):
     e = lambda s: np.roll(line, -s) - np.roll(line, s)     # noqa: E731  (periodic)
     sym = (e(3) - 6 * e(2) + 21 * e(1)) / (12 * h) if ng == 3 else (104 * e(1) - 32 * e(2) + 8 * e(3) - e(4)) / (60 * h)
     assert np.abs((dplus + dminus)[0, 0] - sym).max() <= 1e-12 * np.abs(dplus).max()
+
+
+# ================================================================================================
+# Round-2 pins: parts of the oracle that only GPU-vs-oracle parity used to cover. Each goes through oracle.rhs /
+# oracle.constraints -- the code path the parity tests compare against -- and is compared with something the
+# equations fix: the one-sided stencils of O3 (pinned on their own by P2), closed forms, or numpy linear algebra.
+# ================================================================================================
+def _line_field(p, axis, seed):
+    """random values varying along one axis only (periodic box)"""
+    rng = np.random.default_rng(seed)
+    N = p.N[axis]
+    shape = [1, 1, 1]
+    shape[2 - axis] = N                                   # arrays are [z][y][x]
+    line = rng.uniform(-1.0, 1.0, N).reshape(shape)
+    return np.broadcast_to(line, (p.N[2], p.N[1], p.N[0])).copy()
+
+
+@pytest.mark.parametrize("ng", [3, 4])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("sign", [+1.0, -1.0])
+def test_R2_upwind_side_through_rhs(oracle, ng, axis, sign):
+    """O3 / reading Q9: the advection term beta^k d_k u takes the one-sided stencil on the side the
+    shift points FROM: beta^k >= 0 -> D+ (offsets -1..+3), beta^k < 0 -> its mirror image. Minkowski, KO off, a
+    constant shift along one axis, chi = 1 + eps f: every other term of d_t chi is an exact zero in d-form, so
+    RHS(chi) must equal beta * D^{+-} chi of the stand-alone stencil (pinned by P2 / N1) bit for bit."""
+    p = replace(I.params_noise(12, (1, 1, 1), 0.1), ng=ng, ko_eps=0.0)
+    c = sign * 0.3
+    u = I.minkowski(p)
+    u[I.CHI] += 1e-3 * _line_field(p, axis, 5 + axis)
+    u[I.BETAX + axis] = c
+    r = oracle.rhs(p, u)
+    want = c * oracle.stencil(p, u[I.CHI], 3 if c > 0 else 4, axis)
+    other = c * oracle.stencil(p, u[I.CHI], 4 if c > 0 else 3, axis)
+    assert np.array_equal(r[I.CHI], want)
+    assert np.abs(want - other).max() > 1e-3 * np.abs(want).max()       # the two sides really differ on this data
+
+
+@pytest.mark.parametrize("ng", [3, 4])
+def test_R2_advection_reaches_every_field_with_gauge_switches(oracle, ng):
+    """O5: beta^k d_k u_f enters all 22 right-hand sides, with coefficient 1 except c_adv^alpha on the lapse and
+    c_adv^beta on the shift. Nothing else in F(y) depends on an undifferentiated, spatially constant shift (only
+    -eta beta^i in d_t beta^i), so RHS(beta = c) - RHS(beta = 0) isolates the term for every field."""
+    base = replace(I.params_noise(12, (1, 1, 1), 0.1), ng=ng, ko_eps=0.0, lapse_advect=0.7, shift_advect=0.4,
+                   shift_eta=1.5)
+    c = np.array([0.2, -0.3, 0.25])
+
+    def advection(u, f):
+        """sum_a beta^a D^{sign beta^a}_a u_f with the stand-alone one-sided stencils, side chosen cell by cell"""
+        tot = 0.0
+        for a in range(3):
+            b = u[I.BETAX + a]
+            tot = tot + b * np.where(b >= 0.0, oracle.stencil(base, u[f], 3, a), oracle.stencil(base, u[f], 4, a))
+        return tot
+
+    for f in range(I.NF):
+        u0 = I.minkowski(base)
+        pert = sum(_line_field(base, a, 17 * f + a) for a in range(3))
+        u0[f] += 1e-3 * pert
+        u1 = u0.copy()
+        for a in range(3):
+            u1[I.BETAX + a] += c[a]
+        diff = oracle.rhs(base, u1)[f] - oracle.rhs(base, u0)[f]
+        coef = base.lapse_advect if f == I.ALPHA else (base.shift_advect if f >= I.BETAX else 1.0)
+        want = coef * (advection(u1, f) - advection(u0, f))
+        if f >= I.BETAX:
+            want = want - base.shift_eta * c[f - I.BETAX]
+        scale = np.abs(advection(u1, f)).max()
+        assert scale > 1e-4
+        assert np.abs(diff - want).max() <= 1e-9 * scale, (I.FIELD_NAMES[f], np.abs(diff - want).max() / scale)
+
+
+@pytest.mark.parametrize("ng", [3, 4])
+def test_R2_ko_amplitude_and_coverage_through_rhs(oracle, ng):
+    """PAPER.md:203 ("dissipation 0.5") and O3: Q u = +(eps/64h) [s3 - 6 s2 + 15 s1] per axis (9-point analogue with
+    eps/256h at 6th order) is added to ALL 22 right-hand sides. On the grid-frequency mode (-1)^i the operator's
+    symbol is -eps/h, so RHS(eps) - RHS(0) = -(eps/h) * mode for the perturbed field, whatever else the field does."""
+    p0 = replace(I.params_noise(8, (1, 1, 1), 0.1), ng=ng, ko_eps=0.0)
+    p1 = replace(p0, ko_eps=0.5)                         # the paper's production value
+    i = np.arange(8)
+    mode = np.broadcast_to(((-1.0) ** i)[None, None, :], (8, 8, 8))
+    amp = 1e-6
+    for f in range(I.NF):
+        u = I.minkowski(p0)
+        u[f] += amp * mode
+        diff = oracle.rhs(p1, u) - oracle.rhs(p0, u)
+        want = -(p1.ko_eps / p1.dx) * amp * mode
+        assert np.abs(diff[f] - want).max() <= 1e-8 * np.abs(want).max(), I.FIELD_NAMES[f]
+        others = [g for g in range(I.NF) if g != f]
+        assert np.abs(diff[others]).max() <= 1e-8 * np.abs(want).max()    # dissipation acts field by field
+
+
+def test_R2_momentum_constraint_trace_K_term_and_hamiltonian_theta(oracle):
+    """O5: M_j = ... - 2/3 d_j K with K = Khat + 2 Theta, and H = R - At_ij At^ij + 2/3 K^2. On Minkowski with
+    Theta = a sin(kx) + T0 and Khat = b cos(ky) every other term vanishes: M_x = -(4/3) D_x Theta,
+    M_y = -(2/3) D_y Khat, M_z = 0, H = (2/3)(Khat + 2 Theta)^2, with D the centred stencil (kind 0, pinned by P2)."""
+    p = replace(I.params_noise(16, (1, 1, 1), 0.1), ko_eps=0.0)
+    z, y, x = I.cell_centres(p)
+    L = p.N[0] * p.dx
+    u = I.minkowski(p)
+    u[I.THETA] += 2e-3 * np.sin(2 * np.pi * x / L) + 1e-3 + 0 * y + 0 * z
+    u[I.KHAT] += 3e-3 * np.cos(2 * np.pi * y / L) + 0 * x + 0 * z
+    out, pc = oracle.constraints(p, u, percell=True)
+    dth = oracle.stencil(p, u[I.THETA], 0, 0)
+    dk = oracle.stencil(p, u[I.KHAT], 0, 1)
+    assert np.abs(dth).max() > 5e-3 and np.abs(dk).max() > 5e-3
+    assert np.abs(pc[1] - (-(4.0 / 3.0) * dth)).max() <= 1e-14 * np.abs(dth).max()
+    assert np.abs(pc[2] - (-(2.0 / 3.0) * dk)).max() <= 1e-14 * np.abs(dk).max()
+    assert np.all(pc[3] == 0.0)
+    K = u[I.KHAT] + 2.0 * u[I.THETA]
+    assert np.abs(pc[0] - (2.0 / 3.0) * K * K).max() <= 1e-14 * np.abs(K * K).max()
+
+
+def _sym_matrix(s):
+    """[6][...] packed (xx,xy,xz,yy,yz,zz) -> [...,3,3]"""
+    return np.moveaxis(np.array([[s[0], s[1], s[2]], [s[1], s[3], s[4]], [s[2], s[4], s[5]]]), (0, 1), (-2, -1))
+
+
+def test_R2_Z_norm_closed_form(oracle):
+    """O5: Z^i = Gamt^i - Gamt_d^i and |Z|^2 = gt_ij Z^i Z^j (indices of Z are UP, so the metric, not its inverse).
+    A constant non-diagonal unimodular metric has Gamt_d = 0, hence Z^i = Gamt^i = const and
+    Z_rms = Z_max = sqrt(Z^T gt Z) in closed form."""
+    p = I.params_noise(8, (1, 1, 1), 0.1)
+    A = np.array([[1.7, 0.3, -0.2], [0.3, 0.8, 0.25], [-0.2, 0.25, 1.3]])
+    G = A / np.linalg.det(A) ** (1.0 / 3.0)
+    Zv = np.array([0.4, -0.7, 0.2])
+    u = I.minkowski(p)
+    for q, (a, b) in enumerate(analytic.PAIRS):
+        u[I.GXX + q] = G[a, b]
+    for a in range(3):
+        u[I.GAMX + a] = Zv[a]
+    out = oracle.constraints(p, u)
+    want = math.sqrt(Zv @ G @ Zv)
+    wrong = math.sqrt(Zv @ np.linalg.inv(G) @ Zv)
+    assert abs(want - wrong) > 0.05 * want                     # the data tell the two contractions apart
+    assert abs(out[6] - want) <= 1e-13 * want and abs(out[7] - want) <= 1e-13 * want
+
+
+def test_R2_M_norms_against_numpy(oracle):
+    """O5: |M|^2 = gt^{ij} M_i M_j (indices of M are DOWN, so the inverse metric); M_rms = sqrt(mean |M|^2),
+    M_max = max |M|, rebuilt with numpy from the per-cell M_i on strong-field data (metric far from flat)."""
+    p = I.params_noise(10, (1, 1, 1), 0.05)
+    u, bad = oracle.enforce(p, I.smooth_random_data(p, 21, 0.15))
+    assert bad == 0
+    out, pc = oracle.constraints(p, u, percell=True)
+    G = _sym_matrix(u[I.GXX:I.GZZ + 1])
+    Gi = np.linalg.inv(G)
+    M = np.moveaxis(pc[1:4], 0, -1)
+    m2 = np.einsum("...i,...ij,...j", M, Gi, M)
+    flat = (M ** 2).sum(-1)
+    lowered = np.einsum("...i,...ij,...j", M, G, M)
+    assert abs(np.sqrt(flat.mean()) / np.sqrt(m2.mean()) - 1) > 1e-3       # data distinguish the three norms
+    assert abs(np.sqrt(lowered.mean()) / np.sqrt(m2.mean()) - 1) > 1e-3
+    assert abs(out[2] - np.sqrt(m2.mean())) <= 1e-12 * out[2]
+    assert abs(out[3] - np.sqrt(m2.max())) <= 1e-12 * out[3]
