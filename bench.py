@@ -1,17 +1,22 @@
 #!/usr/bin/env python
 """bench.py -- zone-cycles/s of the fp64 Z4c RK4 step (BASELINE.json `metric`).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference] [--sweep none|point|full]
 
-A "step" is one classical RK4 step (4 stages of RHS -> stage update + enforcement -> ghost fill; by default one
-fused kernel per stage) over the whole pack. Default workload: BASELINE.json configs[1], the linear gravitational wave on 64^3 cells in 64 blocks of
-16^3 (+3 ghosts). One JSON line is printed by rank 0. See DESIGN.md "Measurement" for every figure's definition.
+A "step" is one classical RK4 step (4 stages of RHS -> stage update + enforcement -> ghost fill; by default ONE fused
+kernel per stage) over the whole pack. Default workload: BASELINE.json configs[3], the two-puncture grid of 256^3 cells
+in 512 blocks of 32^3 (+3 ghosts) -- the largest fixed-size configuration; configs[4]'s saturated pack (512 blocks of
+64^3, 133 GB on the device) is timed in the same run and reported under "sweep" with its own clocks record.
+The timed region is K steps, repeated --repeats times (default 5); the line reports the MEDIAN repeat.
+One JSON line is printed by rank 0. See DESIGN.md "Measurement" for every figure's definition.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -32,10 +37,7 @@ RHS_FLOPS_PER_CELL_O6 = 8059      # same census with the 6th-order stencil set (
 # doubles moved per cell and RK4 step by the O6 recurrence: 616, plus the ghost fill
 STEP_DOUBLES_PER_CELL = 616
 GHOST_DOUBLES_PER_GHOST_CELL_STEP = 4 * 22 * 2
-# K2 alone, per launch: reads y (22), writes P (22); stages 3-4 also read P (22)
-RHS_DOUBLES_PER_CELL = (44 + 44 + 66 + 66) / 4.0
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12   # 148 SMs x 64 DFMA/clk x 2 flop x max SM clock
-
 
 WORKLOAD_LABELS = {
     "linear_wave_64": "configs[1]: linear wave 64^3 = 64 blocks of 16^3 (+3 ghosts), periodic",
@@ -43,22 +45,29 @@ WORKLOAD_LABELS = {
     "bbh_256": "configs[3]: two punctures 256^3 = 512 blocks of 32^3, outflow-copy",
     "linear_wave_o6_256": "NEXT-1 / paper Table 1 shape: linear wave 256^3 = 64 blocks of 64^3 (+4 ghosts), 6th order",
 }
-# the paper's own figure for the Table 1 workload (A100, 64^3 blocks, VRAM filled, 6th order + RK4):
-# another machine, context only
-PAPER_A100_ZCPS = 1.36e7
+DEFAULT_WORKLOAD = "bbh_256"
+# configs[4] load sweep: (n, block lattice). "point" = the saturated pack only; "full" = every row.
+SWEEP_POINT = [(64, (8, 8, 8))]
+SWEEP_FULL = [(16, (2, 2, 2)), (16, (4, 4, 4)), (16, (8, 8, 8)), (16, (16, 16, 16)), (16, (24, 24, 24)),
+              (32, (2, 2, 2)), (32, (4, 4, 4)), (32, (8, 8, 8)), (32, (12, 12, 12)), (32, (16, 16, 12)),
+              (64, (2, 2, 2)), (64, (4, 4, 4)), (64, (6, 6, 6)), (64, (8, 8, 8))]
+# the paper's own figure for its Table 1 workload: another machine and 6th order -- context, never a ratio
+PAPER_CONTEXT = {"zcps": 1.36e7, "hardware": "NVIDIA A100", "workload": "linear wave, 64^3 blocks, VRAM filled, "
+                 "6th order + RK4, whole application", "source": "PAPER.md:269 (Table 1)",
+                 "gpu_over_cpu_core": ">~200x (PAPER.md:15, 283)"}
 
 
 def workload(name: str):
-    """(params, initial data, label). Inputs are synthetic and seeded."""
+    """(params, initial data on the host, label). Inputs are synthetic and seeded."""
     if name == "linear_wave_64":
         p = I.params_linear_wave(64, 16)
-        return p, I.linear_wave_data(p), "configs[1]: linear wave 64^3 = 64 blocks of 16^3 (+3 ghosts), periodic"
+        return p, I.linear_wave_data(p), WORKLOAD_LABELS[name]
     if name == "puncture_128":
         p, u, _ = I.config(2)
-        return p, u, "configs[2]: single puncture 128^3 = 64 blocks of 32^3, outflow-copy"
+        return p, u, WORKLOAD_LABELS[name]
     if name == "bbh_256":
         p, u, _ = I.config(3)
-        return p, u, "configs[3]: two punctures 256^3 = 512 blocks of 32^3, outflow-copy"
+        return p, u, WORKLOAD_LABELS[name]
     if name == "linear_wave_o6_256":
         p = replace(I.params_linear_wave(256, 64), ng=4)
         return p, I.linear_wave_data(p), WORKLOAD_LABELS[name]
@@ -71,11 +80,15 @@ def workload(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
-def profiled_traffic(name: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+def profile_record(name: str, ng: int):
+    """What the committed ncu capture of the dominant kernel says for this workload (profiles/r02_traffic.json,
+    written from `ncu --set full` with the commit it was taken at), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
-            return float(json.load(f)[name]["mean_bytes_per_launch"])
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as f:
+            d = json.load(f)
+        rec = dict(d[name])
+        rec["commit"] = d.get("commit")
+        return rec
     except Exception:
         return None
 
@@ -147,8 +160,8 @@ class ClockSampler:
 
 
 def aggregate(local_ms: float, local_units: float, dist=None):
-    """Whole-job figures from per-rank ones: time = MAX over ranks, units = SUM over ranks
-    (replicas: no data-path collective). Works on gloo (CPU tensors) and nccl."""
+    """Whole-job figures from per-rank ones: time = MAX over ranks, units = SUM over ranks.
+    Works on gloo (CPU tensors) and nccl."""
     if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
         return local_ms, local_units
     import torch
@@ -163,8 +176,8 @@ def aggregate(local_ms: float, local_units: float, dist=None):
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
 # ------------------------------------------------------------------------------------------------
-def oracle_sample(name: str):
-    """A bounded sample of the workload with identical per-cell arithmetic."""
+def oracle_sample(name: str, small: bool = False):
+    """A bounded sample of the workload with identical per-cell arithmetic. `small`: a quarter of it (1-thread leg)."""
     if name == "linear_wave_64":
         p = I.params_linear_wave(64, 16)
         ps = replace(p, nb=(4, 1, 1))   # 64 x 16 x 16 periodic slab of the same wave
@@ -173,32 +186,47 @@ def oracle_sample(name: str):
         ps = replace(I.params_linear_wave(256, 16), nb=(16, 1, 1), ng=4)
         return ps, I.linear_wave_data(ps), "256x16x16 periodic slab of the 256^3 wave, 6th-order stencils"
     if name in ("puncture_128", "bbh_256"):
-        p, u, _ = I.config(2 if name == "puncture_128" else 3)
-        lo = p.N[0] // 2 - 16
-        ps = replace(p, n=32, nb=(1, 1, 1))
-        return ps, np.ascontiguousarray(u[:, lo:lo + 32, lo:lo + 32, lo:lo + 32]), "central 32^3 sub-box (clamped edges)"
+        # the 32^3 block next to the puncture at x = +3 (bbh) / at the origin, cut out of the full-size data by its
+        # closed form (no 3 GB array): same dx, same fields, clamped edges
+        full = I.params_puncture(128, 32, 16.0, 2.0) if name == "puncture_128" else I.params_puncture(256, 32, 24.0, 1.0)
+        w = 16 if small else 32
+        centre = (0.0, 0.0, 0.0) if name == "puncture_128" else (3.0, 0.0, 0.0)
+        lo = tuple(c - 0.5 * w * full.dx for c in centre)
+        ps = replace(full, n=w, nb=(1, 1, 1), xmin=lo)
+        if name == "puncture_128":
+            us = I.puncture_data(ps)
+        else:
+            us = I.puncture_data(ps, (0.5, 0.5), ((3.0, 0.0, 0.0), (-3.0, 0.0, 0.0)))
+        return ps, us, f"{w}^3 sub-box around the puncture at {centre} (same dx and data, clamped edges)"
     p, u, _ = workload(name)
     ps = replace(p, nb=(2, 1, 1))
     return ps, I.noise_data(ps, 1000), f"2 blocks of {p.n}^3 of the noise pack"
 
 
-def time_oracle(name: str, steps: int, warmup: int, budget_s: float):
+def time_oracle(name: str, steps: int, warmup: int, budget_s: float, threads: int = 0):
     from oracle import oracle as O
     O.build()
-    ps, us, what = oracle_sample(name)
-    us, _ = O.enforce(ps, us)
-    cores = O.num_threads()
-    t0 = time.perf_counter()
-    u1, _ = O.step(ps, us, 1)                      # calibration step (counts as warm-up)
-    t1 = time.perf_counter() - t0
-    for _ in range(max(0, warmup - 1)):
-        if (time.perf_counter() - t0) > budget_s * 0.25:
-            break
-        O.step(ps, us, 1)
-    k = max(1, min(steps, int(budget_s / max(t1, 1e-6))))
-    t0 = time.perf_counter()
-    O.step(ps, us, k)
-    dt = time.perf_counter() - t0
+    all_threads = O.num_threads()
+    if threads:
+        O.set_num_threads(threads)
+    try:
+        ps, us, what = oracle_sample(name, small=(threads == 1))
+        us, _ = O.enforce(ps, us)
+        cores = O.num_threads()
+        t0 = time.perf_counter()
+        O.step(ps, us, 1)                      # calibration step (counts as warm-up)
+        t1 = time.perf_counter() - t0
+        for _ in range(max(0, warmup - 1)):
+            if (time.perf_counter() - t0) > budget_s * 0.25:
+                break
+            O.step(ps, us, 1)
+        k = max(1, min(steps, int(budget_s / max(t1, 1e-6))))
+        t0 = time.perf_counter()
+        O.step(ps, us, k)
+        dt = time.perf_counter() - t0
+    finally:
+        if threads:
+            O.set_num_threads(all_threads)
     return {"zcps": ps.ncells * k / dt, "cores": cores, "steps": k, "ms_per_step": dt / k * 1e3,
             "sample": f"{what}; {ps.ncells} cells x {k} RK4 steps"}
 
@@ -224,6 +252,64 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
+def timed_steps(sim, K: int, W: int, R: int, barrier, device_index: int):
+    """W warm-up steps, then R repeats of exactly K steps, each bracketed by barrier + synchronize and timed with
+    CUDA events on the library's stream; clocks sampled over all repeats. Returns per-repeat ms and the clocks."""
+    import torch
+    sim.step(W)
+    sim.sync()
+    sampler = ClockSampler(device_index)
+    times = []
+    barrier()
+    sampler.start()
+    for _ in range(R):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(sim.stream)
+        sim.step(K)
+        e1.record(sim.stream)
+        barrier()
+        times.append(e0.elapsed_time(e1))
+    clocks = sampler.stop()
+    sim.sync()                                   # raises if the device error flag is set
+    return times, clocks
+
+
+def sweep_rows(Z, points, K, W, R, device_index, budget_gb):
+    """BASELINE.json configs[4]: Minkowski + seeded 1e-10 noise, periodic; the pack is filled ON THE DEVICE by tiling a
+    2x2x2-block seeded problem, so host memory never holds more than the small tile. Device-resident timing only."""
+    import ctypes as C
+    import torch
+    rows = []
+    lib = Z.load_library()
+    for n, nb in points:
+        p = I.params_noise(n, nb, 0.1)
+        cp = Z.make_params(p)
+        gb = (lib.z4c_state_bytes(C.byref(cp)) + lib.z4c_workspace_bytes(C.byref(cp)) + I.NF * p.ncells * 8) / 1e9
+        free = torch.cuda.mem_get_info()[0] / 1e9
+        if gb > min(budget_gb, free - 4.0):
+            rows.append({"n": n, "blocks": list(nb), "skipped": f"needs {gb:.0f} GB, {free:.0f} GB free"})
+            continue
+        tile = (2, 2, 2)
+        base = torch.from_numpy(I.noise_data(replace(p, nb=tile), 1000)).cuda()
+        u = base.repeat(1, nb[2] // 2, nb[1] // 2, nb[0] // 2).contiguous()
+        sim = Z.Z4c(p, device=f"cuda:{device_index}")
+        sim.use_graph(True)
+        sim.set_initial_data(u)
+        del u, base
+        torch.cuda.empty_cache()
+        times, clocks = timed_steps(sim, K, W, R, torch.cuda.synchronize, device_index)
+        ms = float(np.median(times))
+        dev = float(abs(sim.state[I.CHI, 0, 3:-3, 3:-3, 3:-3] - 1.0).max())
+        rows.append({"n": n, "blocks": list(nb), "cells_per_gpu": p.ncells, "device_gb": round(gb, 1),
+                     "ms_per_step": ms / K, "zcps": p.ncells * K / (ms * 1e-3), "steps": K, "repeats": len(times),
+                     "max_abs_chi_minus_1": dev, "effective_mode": list(sim.effective_mode()), "clocks": clocks})
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -243,7 +329,8 @@ def run_ours(args):
     sim.set_variant(args.variant)
     sim.set_fused(args.fuse)
     sim.use_graph(not args.no_graph)
-    K, W = args.steps, max(args.warmup, 3)
+    eff_variant, eff_fused = sim.effective_mode()
+    K, W, R = args.steps, max(args.warmup, 3), max(args.repeats, 1)
     ncells = p.ncells
 
     def barrier():
@@ -251,49 +338,39 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident throughput ---------------------------------------------------------
+    # ---- device-resident throughput: median of R repeats of exactly K steps ---------------------------
     sim.set_initial_data(u0)
-    sim.step(W)
-    sim.sync()
     l0 = sim.launch_count()
-    sampler = ClockSampler(local_rank)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    sampler.start()
-    with torch.cuda.stream(sim.stream):
-        e0.record(sim.stream)
-        sim.step(K)
-        e1.record(sim.stream)
-    barrier()
-    clocks = sampler.stop()
-    ms_local = e0.elapsed_time(e1)
-    launches = sim.launch_count() - l0
-    sim.sync()                                            # raises if the device error flag is set
+    times, clocks = timed_steps(sim, K, W, R, barrier, local_rank)
+    launches_per_step = (sim.launch_count() - l0) // (W + K * R)
+    ms_local = float(np.median(times))
     ms, units = aggregate(ms_local, float(ncells) * K, dist if world > 1 else None)
     zcps = units / (ms * 1e-3)
 
-    # ---- per-kernel times over the same K steps (events between kernels, no graph) -------------
+    # ---- per-kernel share of the step (events between kernels, no graph) ------------------------------
+    Kt = max(2, min(K, 10))
     sim.step_timed(2)
-    kt = sim.step_timed(K)
-    rhs_ms = kt["rhs"] / (4 * K)
+    kt = sim.step_timed(Kt)
+    total_kt = kt["rhs"] + kt["update"] + kt["ghost"]
     fp64_peak = sim.probe_fp64()
     hbm_peak, hbm_src = measured_peaks()
     flops_cell = RHS_FLOPS_PER_CELL if p.ng == 3 else RHS_FLOPS_PER_CELL_O6
+    # dominant kernel = the RHS / fused stage kernel, 4 launches per step; its launch time from the graph-replayed
+    # step itself when it is the whole step (one kernel per stage), else from the event-separated run
+    rhs_ms = (ms_local / K / 4.0) if eff_fused == 2 else kt["rhs"] / (4 * Kt)
     rhs_tflops = flops_cell * ncells / (rhs_ms * 1e-3) * 1e-12
-    rhs_gbs = RHS_DOUBLES_PER_CELL * 8 * ncells / (rhs_ms * 1e-3) * 1e-9
     g = p.ng
     ghost_cells = p.nblocks * ((p.n + 2 * g) ** 3 - p.n ** 3)
     step_bytes = (STEP_DOUBLES_PER_CELL * ncells + GHOST_DOUBLES_PER_GHOST_CELL_STEP * ghost_cells) * 8
-    total_kt = kt["rhs"] + kt["update"] + kt["ghost"]
+    prof = profile_record(args.workload, g)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ------
     h_in = torch.from_numpy(u0).pin_memory()
     h_out = torch.empty_like(h_in).pin_memory()
-    Ke = max(3, min(K, 20))
-    for _ in range(2):
-        sim.set_initial_data(h_in)
-        sim.step(1)
-        sim.get_interior(h_out.numpy())
+    Ke = max(3, min(K, 20)) if u0.nbytes < 1e9 else 3
+    sim.set_initial_data(h_in)
+    sim.step(1)
+    sim.get_interior(h_out.numpy())
     barrier()
     t0 = time.perf_counter()
     for _ in range(Ke):
@@ -303,58 +380,92 @@ def run_ours(args):
     barrier()
     e2e_ms, e2e_units = aggregate((time.perf_counter() - t0) * 1e3, float(ncells) * Ke, dist if world > 1 else None)
     nbytes = int(u0.nbytes)
+    state_mb = (sim.state.numel() + sim.work.numel()) * 8 / 1e6
+    sim.close()
+    del sim, h_in, h_out
+    torch.cuda.empty_cache()
+
+    # ---- configs[4] load sweep (device-resident), each row with its own clocks record -----------------
+    sweep = None
+    if world == 1 and args.sweep != "none" and p.ng == 3:
+        pts = SWEEP_POINT if args.sweep == "point" else SWEEP_FULL
+        sweep = sweep_rows(z4c, pts, min(K, 10) if args.sweep == "point" else min(K, 20), 3, R, local_rank,
+                           args.budget_gb)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        r = time_oracle(args.workload, 1000, 1, budget_s=15.0)
-        cpu = {"value": r["zcps"], "unit": "zone-cycles/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+        r = time_oracle(args.workload, 1000, 1, budget_s=12.0)
+        r1 = time_oracle(args.workload, 1000, 1, budget_s=8.0, threads=1)
+        cpu = {"value": r["zcps"], "unit": "zone-cycles/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+               "single_thread": {"value": r1["zcps"], "unit": "zone-cycles/s", "cores": 1, "sample": r1["sample"]}}
 
     if rank == 0:
         line = {
             "metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": zcps, "unit": "zone-cycles/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": (zcps / PAPER_A100_ZCPS) if args.workload == "linear_wave_o6_256" and world == 1 else None,
-            "dtype": "f64", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": label, "cells_per_gpu": ncells, "blocks": p.nblocks, "n": p.n, "ghosts": g,
                        "parallelism": "replicas" if world > 1 else "1 GPU",
-                       "l2": "no flush: y+P+Q working set %.0f MB > 126 MB L2" %
-                             ((sim.state.numel() + sim.work.numel()) * 8 / 1e6),
-                       "graph": not args.no_graph, "fuse_mode": args.fuse, "rhs_variant": args.variant},
+                       "l2": "no flush: y+y2+P+Q working set %.0f MB > 126 MB L2" % state_mb,
+                       "graph": not args.no_graph, "fuse_mode": eff_fused, "rhs_variant": eff_variant,
+                       "requested": {"fuse_mode": args.fuse, "rhs_variant": args.variant}},
+            "repeats": {"n": R, "ms_per_step_each": [t / K for t in times], "statistic": "median"},
             "clocks": clocks,
             "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": "zone-cycles/s", "h2d_bytes_per_step": nbytes,
                     "d2h_bytes_per_step": nbytes, "steps": Ke,
                     "what": "z4c_set_initial_data(host) + z4c_step(1) + z4c_get_interior(host) per step, pinned"},
-            "gpu_launches": int(launches),
-            "roofline": {"kernel": "k_rhs_tiled<STAGE> (one kernel per RK stage)" if args.fuse == 2 and args.variant != 1 else "K2 z4c_rhs", "bound": "alu", "achieved": rhs_tflops, "peak": fp64_peak,
+            "gpu_launches": int(launches_per_step * K),
+            "roofline": {"kernel": "k_stage<STAGE> (one kernel per RK stage)" if eff_fused == 2 else "K2 z4c_rhs",
+                         "bound": "alu", "achieved": rhs_tflops, "peak": fp64_peak,
                          "unit": "TFLOP/s", "frac": rhs_tflops / fp64_peak,
-                         "traffic": profiled_traffic(args.workload),
+                         "flops_source": "ALGORITHMIC: the oracle's unfused operation census (add = mul = div = 1), "
+                                         "not executed instructions",
+                         "traffic": prof.get("mean_bytes_per_launch") if prof else None,
+                         "traffic_commit": prof.get("commit") if prof else None,
+                         "fp64_pipe_active_pct_ncu": prof.get("fp64_pipe_active_pct") if prof else None,
                          "peak_source": "measured live: z4c_probe_fp64 DFMA loop (nominal %.1f at 1965 MHz)" % FP64_NOMINAL_TFLOPS,
                          "flops_per_cell": flops_cell, "ms_per_launch": rhs_ms,
-                         "hbm_gbs_algorithmic": rhs_gbs, "share_of_step": kt["rhs"] / total_kt},
+                         "timing": "graph-replayed step / 4" if eff_fused == 2 else "events between kernels",
+                         "share_of_step": kt["rhs"] / total_kt},
             "step_roofline": {"bound": "hbm", "achieved": step_bytes * K / (ms_local * 1e-3) * 1e-9, "peak": hbm_peak,
                               "unit": "GB/s", "frac": step_bytes * K / (ms_local * 1e-3) * 1e-9 / hbm_peak,
                               "peak_source": hbm_src, "bytes_per_cell_step": step_bytes / ncells,
-                              "kernel_ms_per_step": {k: v / K for k, v in kt.items()}},
+                              "kernel_ms_per_step": {k: v / Kt for k, v in kt.items()}},
+            "sweep": sweep,
             "cpu_baseline": cpu,
+            "context": {"paper": PAPER_CONTEXT},
         }
         print(json.dumps(line))
-    sim.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=400)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--repeats", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="linear_wave_64")
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--sweep", default="point", choices=["none", "point", "full"])
+    ap.add_argument("--budget-gb", type=float, default=150.0)
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--fuse", type=int, default=2, help="0: K2,K3,K1; 1: K2,K3+push; 2: one kernel per RK stage")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` is a complete command: re-launch under torch.distributed.run, one rank per GPU
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

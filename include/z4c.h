@@ -23,6 +23,11 @@
  *    host-side z4c_ctx and never allocates device memory.
  *  - Stream semantics: every call enqueues its work on the CUDA stream given to z4c_create()
  *    and returns without synchronising, except where stated ("synchronises").
+ *  - Stream ordering of caller-owned DEVICE buffers (on_device = 1 arguments, d_percell, d_out, d_minchi ...):
+ *    the library reads and writes them on ITS stream only and inserts no event against any other stream. A
+ *    caller that produces or consumes such a buffer on another stream must order the two itself: make the
+ *    library's stream wait for the producer before the call, and make the consumer wait for the library's
+ *    stream (or call z4c_sync) after it. The Python binding does exactly this against torch's current stream.
  *  - Determinism: results are bitwise reproducible run to run (no atomics on the state path).
  *
  * State layout (part of the contract so a caller may view the buffer as a tensor):
@@ -144,12 +149,9 @@ int z4c_sync(z4c_ctx* ctx);
 
 /* Number of kernel launches the library has enqueued on this context so far. */
 int64_t z4c_launch_count(const z4c_ctx* ctx);
-/* Select the RHS kernel variant: 0 = tuned kernel, TMA-staged 16x4x2 tiles, 128 threads, 2 CTAs per SM
- * (default); 1 = plain global-memory kernel; 2 = tuned kernel with 16x4x4 tiles, 256 threads, 1 CTA per SM;
- * 3 = persistent one-kernel-per-stage variant (CTAs walk a stream of tiles and prefetch the next tile's halo
- * tiles; experimental, measured slower than variant 0); 4 = variant 0 with the P/Q tiles read by batched global loads
- * instead of TMA and the late-use derivatives parked in shared memory as they are produced (measured 3 % slower).
- * For A/B measurements; all variants compute the same values. */
+/* Select the RHS kernel variant: 0 = tuned kernel with TMA-staged shared-memory tiles (default); 1 = plain
+ * global-memory kernel (the first correct kernel; also what runs when the tuned one is unavailable: odd n).
+ * For A/B measurements; both compute the same values. Other values: Z4C_EINVAL. */
 int z4c_set_variant(z4c_ctx* ctx, int variant);
 /* Enable (1) / disable (0) CUDA-graph replay of the RK4 step inside z4c_step. Default 0. */
 int z4c_use_graph(z4c_ctx* ctx, int enable);
@@ -162,6 +164,12 @@ int z4c_use_graph(z4c_ctx* ctx, int enable);
  * writing the next one to a second buffer kept in the workspace (4 stages: the caller's buffer is current
  * again at the end of every step). Falls back to mode 1 where the tuned K2 is unavailable (odd n, variant 1). */
 int z4c_set_fused(z4c_ctx* ctx, int mode);
+
+/* What actually runs, after fallbacks: *variant = 0 (tuned TMA kernel) or 1 (plain kernel: requested, or n is odd, or
+ * the driver refused a tensor map); *fused = 0, 1 or 2 as in z4c_set_fused (2 needs the tuned kernel, else 1 runs).
+ * Both are host pointers. bench.py reports these, and the GPU tests assert them, so that a silent fallback cannot
+ * pass for the tuned path. */
+int z4c_effective_mode(const z4c_ctx* ctx, int* variant, int* fused);
 
 double z4c_time(const z4c_ctx* ctx);             /* simulation time = steps taken * dt */
 const char* z4c_last_error(const z4c_ctx* ctx);  /* host string owned by the context ("" if none) */

@@ -13,7 +13,6 @@ LIB_NG4 = os.path.join(HERE, "libz4c_ng4.so")    # 4 ghosts, 6th-order stencils 
 LIBS = {3: LIB, 4: LIB_NG4}
 SOURCES = ["z4c_lib.cu"]
 HEADERS = ["z4c_math.cuh", "z4c_rhs.cuh", "z4c_pack.cuh", "z4c_kernels.cuh", "z4c_rhs_tiled.cuh",
-           "z4c_stage_persistent.cuh",
            os.path.join("..", "..", "include", "z4c.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=true", "-Xcompiler", "-fPIC", "--shared", "-cudart", "shared"]

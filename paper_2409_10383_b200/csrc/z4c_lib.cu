@@ -12,7 +12,6 @@
 #include "../../include/z4c.h"
 #include "z4c_kernels.cuh"
 #include "z4c_rhs_tiled.cuh"
-#include "z4c_stage_persistent.cuh"
 
 using namespace z4c;
 
@@ -38,10 +37,8 @@ struct z4c_ctx {
   int graph_launches;
   double* ybuf[2];    // ybuf[0] = y (caller's state), ybuf[1] = second state buffer in the workspace
   CUtensorMap ymap[2];  // TMA descriptors of the two state buffers (tuned K2)
-  CUtensorMap ymap2[2]; // same with the 16x4x4 tile box (variant 2)
-  CUtensorMap ymapP[2]; // state buffers with the persistent kernel's tile box
   int num_sms;
-  RegMaps rmap, rmap2;  // TMA descriptors of the RK registers P, Q for the two tile shapes
+  RegMaps rmap;         // TMA descriptors of the RK registers P, Q
   int have_ymap;
   std::string err;
 };
@@ -155,26 +152,9 @@ cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, const RegMa
     default: return launch_rhs_tiled_t<Cfg, 4>(map, rm, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa);
   }
 }
-template <int STAGE>
-cudaError_t launch_persistent(z4c_ctx* c, int in, const StageArgs& sa) {
-  return launch_stage_persistent_t<StageTile, STAGE>(c->ymapP[in], c->g, c->P, c->fd, c->sp, c->dt, c->stream, sa,
-                                                     c->num_sms);
-}
 int launch_fused_stage(z4c_ctx* c, int stage, int in) {
   StageArgs sa{c->ybuf[in], c->Q, c->ybuf[1 - in], c->prm.chi_floor, c->flag};
-  if (c->variant == 3) {   // persistent kernel (experimental: measured slower, see z4c_stage_persistent.cuh)
-    cudaError_t e = stage == 1 ? launch_persistent<1>(c, in, sa) : stage == 2 ? launch_persistent<2>(c, in, sa)
-                  : stage == 3 ? launch_persistent<3>(c, in, sa) : launch_persistent<4>(c, in, sa);
-    if (e != cudaSuccess) return check_cuda(c, e, "k_stage_persistent launch");
-    return check_launch(c, "k_stage_persistent");
-  }
-  if (c->variant == 4) {
-    cudaError_t e4 = launch_fused_stage_t<RhsTile5>(c, c->ymap[in], c->rmap, stage, sa);
-    if (e4 != cudaSuccess) return check_cuda(c, e4, "k_rhs_tiled launch");
-    return check_launch(c, "k_rhs_tiled<stage>");
-  }
-  cudaError_t e = c->variant == 2 ? launch_fused_stage_t<RhsTile2>(c, c->ymap2[in], c->rmap2, stage, sa)
-                                  : launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);   // variant 0
+  cudaError_t e = launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
   return check_launch(c, "k_rhs_tiled<stage>");
 }
@@ -341,16 +321,13 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
     c->num_sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
   }
+  // The tuned kernels need TMA descriptors (16-byte strides: even n) and their shared-memory opt-in, which is a
+  // per-device attribute: set here, for the current device, for every instantiation this context can launch.
   c->have_ymap = rhs_tiled_supported(c->g) && make_state_tensor_map<RhsTile>(c->g, c->ybuf[0], &c->ymap[0]) &&
                  make_state_tensor_map<RhsTile>(c->g, c->ybuf[1], &c->ymap[1]) &&
-                 make_state_tensor_map<RhsTile2>(c->g, c->ybuf[0], &c->ymap2[0]) &&
-                 make_state_tensor_map<RhsTile2>(c->g, c->ybuf[1], &c->ymap2[1]) &&
-                 make_state_tensor_map<StageTile>(c->g, c->ybuf[0], &c->ymapP[0]) &&
-                 make_state_tensor_map<StageTile>(c->g, c->ybuf[1], &c->ymapP[1]) &&
                  make_register_tensor_map<RhsTile>(c->g, c->P, &c->rmap.p) &&
                  make_register_tensor_map<RhsTile>(c->g, c->Q, &c->rmap.q) &&
-                 make_register_tensor_map<RhsTile2>(c->g, c->P, &c->rmap2.p) &&
-                 make_register_tensor_map<RhsTile2>(c->g, c->Q, &c->rmap2.q) ? 1 : 0;
+                 configure_rhs_tiled<RhsTile>() == cudaSuccess ? 1 : 0;
   cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
   if (e != cudaSuccess) {
     delete c;
@@ -530,7 +507,7 @@ int z4c_sync(z4c_ctx* c) {
 int64_t z4c_launch_count(const z4c_ctx* c) { return c ? c->launches : 0; }
 
 int z4c_set_variant(z4c_ctx* c, int variant) {
-  if (!c || variant < 0 || variant > 4) return Z4C_EINVAL;
+  if (!c || variant < 0 || variant > 1) return Z4C_EINVAL;
   if (variant != c->variant) drop_graph(c);
   c->variant = variant;
   return Z4C_OK;
@@ -548,6 +525,14 @@ int z4c_set_fused(z4c_ctx* c, int enable) {
   if (enable < 0 || enable > 2) return Z4C_EINVAL;
   if (enable != c->fuse_ghosts) drop_graph(c);
   c->fuse_ghosts = enable;
+  return Z4C_OK;
+}
+
+int z4c_effective_mode(const z4c_ctx* c, int* variant, int* fused) {
+  if (!c || !variant || !fused) return Z4C_EINVAL;
+  const bool tuned = c->variant != 1 && c->have_ymap;
+  *variant = tuned ? 0 : 1;
+  *fused = fully_fused(c) ? 2 : (c->fuse_ghosts ? 1 : 0);
   return Z4C_OK;
 }
 

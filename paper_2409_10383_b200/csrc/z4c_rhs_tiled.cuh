@@ -426,22 +426,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   register / state rows and put two tile rows of a warp on the same shared-memory banks.
 #if Z4C_NG == 3
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
-using RhsTile2 = TileCfg<16, 4, 4, 3, 1>;
 #else
 // 4 ghosts: the halo tile grows to 24 x 12 x 10 (23 KB); to keep 2 CTAs per SM the P/Q tiles are read by batched
 // global loads instead of TMA (93 KB of shared memory per CTA)
 using RhsTile = TileCfg<16, 4, 2, 3, 2, false, false>;
-using RhsTile2 = TileCfg<16, 4, 4, 3, 1, false, false>;
 #endif
-// variant 4: P/Q by batched global loads + early parking. Measured 0.189 ms per launch at 64^3 against 0.183 ms for the
-// default; with the freed shared memory spent on a 5-deep ring instead it was 0.187 ms: neither the late tiles nor the
-// register pressure of the field stream is what limits the default kernel.
-#if Z4C_NG == 3
-using RhsTile5 = TileCfg<16, 4, 2, 3, 2, false>;
-#else
-using RhsTile5 = RhsTile;
-#endif
-
 inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA strides must be 16-byte multiples
 
 // Encode the 5-D tensor map (i, j, k, block, field) of the state pack with a halo-tile box. Returns false if
@@ -491,21 +480,31 @@ inline bool make_register_tensor_map(const Pack& g, const double* reg, CUtensorM
 
 struct RegMaps { CUtensorMap p, q; };
 
+// Shared-memory opt-in of every stage instantiation, for the CURRENT device (function attributes are per device:
+// z4c_create calls this once per context, so a process may drive several devices).
+template <class Cfg, int STAGE>
+inline cudaError_t configure_rhs_tiled_stage() {
+  constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
+  cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                              cudaSharedmemCarveoutMaxShared);
+}
+template <class Cfg>
+inline cudaError_t configure_rhs_tiled() {
+  cudaError_t e = configure_rhs_tiled_stage<Cfg, 0>();
+  if (e == cudaSuccess) e = configure_rhs_tiled_stage<Cfg, 1>();
+  if (e == cudaSuccess) e = configure_rhs_tiled_stage<Cfg, 2>();
+  if (e == cudaSuccess) e = configure_rhs_tiled_stage<Cfg, 3>();
+  if (e == cudaSuccess) e = configure_rhs_tiled_stage<Cfg, 4>();
+  return e;
+}
+
 template <class Cfg, int STAGE>
 inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm, const Pack& g, double* P, const FdConst& fd,
                                       const SrcParams& sp, double coef, double dt, cudaStream_t st,
                                       const StageArgs& sa) {
-  static bool attr_set = false;
   constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         smem);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                             cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
   const long long nblocks = (long long)tx * ty * tz * g.nblk;
   if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;

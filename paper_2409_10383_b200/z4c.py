@@ -22,7 +22,7 @@ LIB_PATH_NG4 = os.path.join(_HERE, "libz4c_ng4.so")    # built with 4 ghost zone
 SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_initial_data", "z4c_step",
            "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
            "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
-           "z4c_probe_fp64", "z4c_time",
+           "z4c_probe_fp64", "z4c_effective_mode", "z4c_time",
            "z4c_last_error", "z4c_destroy"]
 
 
@@ -86,6 +86,7 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_set_fused.argtypes = [vp, C.c_int]
     L.z4c_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.z4c_probe_fp64.argtypes = [vp, vp, C.c_int, C.POINTER(C.c_double)]
+    L.z4c_effective_mode.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.z4c_time.argtypes = [vp]
     L.z4c_time.restype = C.c_double
     L.z4c_last_error.argtypes = [vp]
@@ -94,7 +95,7 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_destroy.restype = None
     for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior",
                "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
-               "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64"):
+               "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64", "z4c_effective_mode"):
         getattr(L, fn).restype = C.c_int
     if path == default:
         _libs[ng] = L
@@ -144,6 +145,21 @@ class Z4c:
         if rc != 0:
             raise Z4cError(rc, self.lib.z4c_last_error(self.h).decode())
 
+    def _before(self, *tensors):
+        """Order the library's stream after the caller's current stream before a call that reads or writes a
+        caller-owned device tensor (stream-ordering contract of include/z4c.h)."""
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)
+            for t in tensors:
+                t.record_stream(self.stream)      # the caching allocator must not reuse it while we still run
+
+    def _after(self):
+        """... and the caller's current stream after the library's, so the caller may consume the result."""
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            cur.wait_stream(self.stream)
+
     @property
     def interior_shape(self):
         N = self.p.N
@@ -162,7 +178,9 @@ class Z4c:
                 t = interior
                 assert t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == self.interior_shape
                 if t.is_cuda:
+                    self._before(t)
                     self._check(self.lib.z4c_set_initial_data(self.h, t.data_ptr(), 1))
+                    self._after()
                 else:
                     self._check(self.lib.z4c_set_initial_data(self.h, t.data_ptr(), 0))
 
@@ -176,7 +194,8 @@ class Z4c:
         with self.torch.cuda.device(self.device):
             if percell:
                 pc = self.torch.empty((4,) + self.interior_shape[1:], dtype=self.torch.float64, device=self.device)
-            self._check(self.lib.z4c_constraints(self.h, out, pc.data_ptr() if percell else None))
+                self._before(pc)
+            self._check(self.lib.z4c_constraints(self.h, out, pc.data_ptr() if percell else None))   # synchronises
         res = np.array(list(out))
         return (res, pc.cpu().numpy()) if percell else res
 
@@ -188,6 +207,7 @@ class Z4c:
             mn = torch.empty(nblk, dtype=torch.float64, device=self.device)
             mx = torch.empty(nblk, dtype=torch.float64, device=self.device)
             fl = torch.empty(nblk, dtype=torch.int32, device=self.device)
+            self._before(mn, mx, fl)
             self._check(self.lib.z4c_refine_indicators(self.h, float(chi_min), float(dchi_max), mn.data_ptr(),
                                                        mx.data_ptr(), fl.data_ptr()))
             self._check(self.lib.z4c_sync(self.h))
@@ -198,7 +218,9 @@ class Z4c:
         with self.torch.cuda.device(self.device):
             if out is not None and not isinstance(out, np.ndarray):
                 assert out.is_cuda and out.dtype == self.torch.float64 and out.is_contiguous()
+                self._before(out)
                 self._check(self.lib.z4c_get_interior(self.h, out.data_ptr(), 1))
+                self._after()
                 return out
             a = out if out is not None else np.empty(self.interior_shape, dtype=np.float64)
             assert a.flags["C_CONTIGUOUS"] and a.dtype == np.float64 and a.shape == self.interior_shape
@@ -212,6 +234,7 @@ class Z4c:
     def eval_rhs(self) -> np.ndarray:
         with self.torch.cuda.device(self.device):
             out = self.torch.empty(self.interior_shape, dtype=self.torch.float64, device=self.device)
+            self._before(out)
             self._check(self.lib.z4c_eval_rhs(self.h, out.data_ptr()))
             self._check(self.lib.z4c_sync(self.h))
         return out.cpu().numpy()
@@ -229,6 +252,12 @@ class Z4c:
 
     def set_variant(self, v: int):
         self._check(self.lib.z4c_set_variant(self.h, int(v)))
+
+    def effective_mode(self):
+        """z4c_effective_mode: (variant, fused) that actually run after fallbacks."""
+        v, f = C.c_int(), C.c_int()
+        self._check(self.lib.z4c_effective_mode(self.h, C.byref(v), C.byref(f)))
+        return int(v.value), int(f.value)
 
     def use_graph(self, enable: bool):
         self._check(self.lib.z4c_use_graph(self.h, int(bool(enable))))

@@ -53,6 +53,32 @@ def test_workload_table_matches_baseline_configs():
     assert ps.N == (64, 16, 16)
 
 
+def test_default_workload_is_the_largest_fixed_config():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.DEFAULT_WORKLOAD == "bbh_256" and "configs[3]" in bench.WORKLOAD_LABELS["bbh_256"]
+    ps, us, what = bench.oracle_sample("bbh_256")
+    assert ps.N == (32, 32, 32) and abs(ps.dx - 48.0 / 256) < 1e-15 and ps.bc == 1 and ps.shift_eta == 1.0
+    assert us[0].min() < 0.05                      # the sample really contains the puncture (chi -> 0)
+    ps1, _, _ = bench.oracle_sample("bbh_256", small=True)
+    assert ps1.N == (16, 16, 16)
+    assert (64, (8, 8, 8)) in bench.SWEEP_POINT and len(bench.SWEEP_FULL) >= 12
+
+
+def test_gpus_flag_spawns_the_ranks_itself():
+    """`python bench.py --gpus 2` must be a complete command (it re-launches itself under torch.distributed.run,
+    127.0.0.1 rendezvous). Checked on the CPU-only reference arm: rank 0 prints the one line, rank 1 exits 0 silently."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                          "--steps", "1", "--warmup", "1", "--workload", "linear_wave_64"],
+                         capture_output=True, text=True, timeout=900, cwd=ROOT, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    line = json.loads(lines[0])
+    assert line["impl"] == "reference" and line["n_gpus"] == 2
+
+
 def test_reference_arm_prints_contract_line():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
                           "--warmup", "1"], capture_output=True, text=True, timeout=600, cwd=ROOT)

@@ -118,6 +118,58 @@ def test_config4_two_punctures_256_full(Z, oracle):
     sim.close()
 
 
+@pytest.mark.parametrize("ng", [3, 4])
+def test_one_64_cubed_block_against_the_oracle(Z, oracle, ng):
+    """n = 64 is the paper's Table-1 block shape and the largest block of configs[4]: one periodic block
+    with strong-field data, compared with the oracle element by element after 1 step (1e-12) and, at 4th order, after
+    5 steps (1e-10). 64 = 4 x 16 tiles along x, 16 along y, 32 along z: every tile position of a block is covered."""
+    p = replace(I.params_noise(64, (1, 1, 1), dx=0.02), ng=ng)
+    u = I.smooth_random_data(p, 13, 0.1)
+    sim = Z.Z4c(p)
+    sim.use_graph(True)
+    sim.set_initial_data(u)
+    assert sim.effective_mode() == (0, 2)
+    ref = oracle.enforce(p, u)[0]
+    for target, tol in ((1, 1e-12), (5, 1e-10)) if ng == 3 else ((1, 1e-12),):
+        done = int(round(sim.time() / p.dt))
+        ref, bad = oracle.step(p, ref, target - done)
+        assert bad == 0
+        sim.step(target - done)
+        sim.sync()
+        got = sim.get_interior()
+        err = rel_err(got, ref, perturbation_scale(ref, p))
+        assert err.max() <= tol, (target, dict(zip(I.FIELD_NAMES, err)))
+    sim.close()
+
+
+def test_two_64_cubed_blocks_outflow_subboxes(Z, oracle):
+    """a 2 x 1 x 1 pack of 64^3 blocks with the outflow-copy boundary: block face, physical corner and interior sub-boxes"""
+    p = replace(I.params_noise(64, (2, 1, 1), dx=0.02), bc=1, shift_eta=1.0)
+    u = I.smooth_random_data(p, 17, 0.1)
+    sim = run(Z, p, u, 1)
+    got = sim.get_interior()
+    half = 8
+    w = 2 * (half + DEP)
+    N = p.N
+    for c in [(64, 32, 32), (0, 0, 0), (127, 63, 10), (63, 20, 63)]:
+        lo = [min(max(c[a] - half - DEP, 0), N[a] - w) for a in range(3)]
+        sub = np.ascontiguousarray(u[:, lo[2]:lo[2] + w, lo[1]:lo[1] + w, lo[0]:lo[0] + w])
+        ps = replace(p, n=w, nb=(1, 1, 1))
+        ref, bad = oracle.step(ps, oracle.enforce(ps, sub)[0], 1)
+        assert bad == 0
+        sl = []
+        for a in range(3):
+            a0 = 0 if lo[a] == 0 else DEP
+            a1 = w if lo[a] + w == N[a] else w - DEP
+            sl.append(slice(a0, a1))
+        r = ref[:, sl[2], sl[1], sl[0]]
+        g = got[:, lo[2] + sl[2].start:lo[2] + sl[2].stop, lo[1] + sl[1].start:lo[1] + sl[1].stop,
+                lo[0] + sl[0].start:lo[0] + sl[0].stop]
+        err = rel_err(g, r, perturbation_scale(ref, ps))
+        assert err.max() <= 1e-12, (c, dict(zip(I.FIELD_NAMES, err)))
+    sim.close()
+
+
 @pytest.mark.parametrize("n,nb", [(16, (8, 8, 8)), (32, (4, 4, 2)), (64, (2, 2, 2))])
 def test_config5_periodic_tiling_invariance(Z, oracle, n, nb):
     tile = (2, 2, 2) if n < 64 else (1, 1, 1)
