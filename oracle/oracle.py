@@ -27,7 +27,7 @@ class _OParams(C.Structure):
 
 def build(force: bool = False) -> str:
     """Compile liboz4c.so with the system g++ (-O2 -ffp-contract=off -fopenmp)."""
-    srcs = [os.path.join(_HERE, f) for f in ("z4c_oracle.cpp", "z4c_physics.hpp", "z4c_oracle.hpp")]
+    srcs = [os.path.join(_HERE, f) for f in ("z4c_oracle.cpp", "z4c_physics.hpp", "z4c_oracle.hpp", "z4c_amr.hpp")]
     if (not force and os.path.exists(_LIB_PATH)
             and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(s) for s in srcs)):
         return _LIB_PATH
@@ -63,6 +63,16 @@ def lib():
         L.oz4c_count_flops.argtypes = [pp, dp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
         L.oz4c_refine_indicators.argtypes = [pp, dp, C.c_int, dp, dp]
         L.oz4c_num_threads.restype = C.c_int
+        ip = C.POINTER(C.c_int32)
+        L.oz4c_lagrange_weights.argtypes = [C.c_int, dp, C.c_double, dp]
+        L.oz4c_restrict_weights.argtypes = [C.c_int, C.c_int, C.c_int, dp]
+        L.oz4c_restrict_weights.restype = C.c_int
+        L.oz4c_prolong_weights.argtypes = [C.c_int, C.c_int, dp]
+        L.oz4c_prolong_weights.restype = C.c_int
+        L.oz4c_restrict.argtypes = [C.c_int, C.c_int, ip, dp, dp, C.c_int]
+        L.oz4c_prolong.argtypes = [C.c_int, ip, C.c_int, ip, dp, ip, ip, dp, C.c_int]
+        L.oz4c_step_two_level.argtypes = [pp, pp, C.c_int, ip, dp, dp, C.c_int]
+        L.oz4c_step_two_level.restype = C.c_int
         L.oz4c_set_num_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
@@ -171,3 +181,58 @@ def count_flops(p, u: np.ndarray, i: int, j: int, k: int):
     lib().oz4c_count_flops(C.byref(_op(p, _N_of(u))), _ptr(u), i, j, k, cnt)
     return {"rhs": {"add": cnt[0], "mul": cnt[1], "div": cnt[2]},
             "constraints": {"add": cnt[3], "mul": cnt[4], "div": cnt[5]}}
+
+
+# ---- NEXT-3: restriction / prolongation at a factor-2 refinement boundary ----------------
+def _i3(v):
+    return (C.c_int32 * 3)(int(v[0]), int(v[1]), int(v[2]))
+
+
+def lagrange_weights(xs, x: float) -> np.ndarray:
+    """Eq. (1), PAPER.md:104."""
+    xs = np.ascontiguousarray(xs, dtype=np.float64)
+    w = np.empty_like(xs)
+    lib().oz4c_lagrange_weights(len(xs), _ptr(xs), float(x), _ptr(w))
+    return w
+
+
+def restrict_weights(Il: int, ng: int, nf: int):
+    """(first fine node, weights) of the restriction stencil of local coarse node Il in a fine block of nf cells."""
+    w = np.empty(ng + 1)
+    s = lib().oz4c_restrict_weights(int(Il), int(ng), int(nf), _ptr(w))
+    return s, w
+
+
+def prolong_weights(i: int, ng: int):
+    """(first coarse node, weights) of the prolongation stencil of fine node i (relative to the region corner)."""
+    w = np.empty(ng + 1)
+    s = lib().oz4c_prolong_weights(int(i), int(ng), _ptr(w))
+    return s, w
+
+
+def restrict(fine: np.ndarray, ng: int, nf: int) -> np.ndarray:
+    """fine [F][Nz][Ny][Nx] (active cells of the fine region, blocks of nf^3) -> coarse [F][Nz/2][Ny/2][Nx/2]."""
+    fine = np.ascontiguousarray(fine, dtype=np.float64)
+    F, Nz, Ny, Nx = fine.shape
+    out = np.empty((F, Nz // 2, Ny // 2, Nx // 2))
+    lib().oz4c_restrict(int(ng), int(nf), _i3((Nx, Ny, Nz)), _ptr(fine), _ptr(out), F)
+    return out
+
+
+def prolong(coarse: np.ndarray, ng: int, bc: int, origin, lo, hi) -> np.ndarray:
+    """coarse [F][Ncz][Ncy][Ncx] -> values on the fine index box [lo, hi) (x, y, z; relative to the corner of the
+    fine region, which is the coarse cell `origin`), returned as [F][hz-lz][hy-ly][hx-lx]."""
+    coarse = np.ascontiguousarray(coarse, dtype=np.float64)
+    F, Nz, Ny, Nx = coarse.shape
+    out = np.empty((F, hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0]))
+    lib().oz4c_prolong(int(ng), _i3((Nx, Ny, Nz)), int(bc), _i3(origin), _ptr(coarse), _i3(lo), _i3(hi), _ptr(out), F)
+    return out
+
+
+def step_two_level(pc, pf, nf: int, origin, uc: np.ndarray, uf: np.ndarray, nsteps: int):
+    """Two-level RK4 steps (coarse level everywhere, fine box at coarse cell `origin`); returns (uc, uf, bad)."""
+    uc = np.array(uc, dtype=np.float64, order="C", copy=True)
+    uf = np.array(uf, dtype=np.float64, order="C", copy=True)
+    bad = lib().oz4c_step_two_level(C.byref(_op(pc, _N_of(uc))), C.byref(_op(pf, _N_of(uf))), int(nf), _i3(origin),
+                                    _ptr(uc), _ptr(uf), int(nsteps))
+    return uc, uf, bad

@@ -8,6 +8,7 @@
 // IEEE-754 binary64 operation, in the order written).  Optional OpenMP over z-planes.
 // =====================================================================================
 #include "z4c_physics.hpp"
+#include "z4c_amr.hpp"
 
 #include <cmath>
 #include <cstring>
@@ -41,11 +42,15 @@ static inline int map_index(int i, int N, int bc) {
 
 struct View {
   const Params& P;
-  const double* u;       // [NF][Nz][Ny][Nx]
+  const double* u;       // [NF][Nz][Ny][Nx]; with pad > 0: [NF][Nz+2pad][Ny+2pad][Nx+2pad]
   size_t ncell;
-  View(const Params& p, const double* uu) : P(p), u(uu),
-      ncell((size_t)p.N[0] * p.N[1] * p.N[2]) {}
+  int pad;               // 0: neighbours by wrap/clamp (O2); > 0: the array carries `pad` filled ghost layers (NEXT-3:
+                         // the fine level of a refinement boundary, whose ghosts come from prolongation)
+  View(const Params& p, const double* uu, int pad_ = 0) : P(p), u(uu),
+      ncell((size_t)(p.N[0] + 2 * pad_) * (p.N[1] + 2 * pad_) * (p.N[2] + 2 * pad_)), pad(pad_) {}
   inline double at(int f, int i, int j, int k) const {
+    if (pad > 0)
+      return u[(size_t)f * ncell + ((size_t)(k + pad) * (P.N[1] + 2 * pad) + (j + pad)) * (P.N[0] + 2 * pad) + (i + pad)];
     i = map_index(i, P.N[0], P.bc); j = map_index(j, P.N[1], P.bc); k = map_index(k, P.N[2], P.bc);
     return u[(size_t)f * ncell + ((size_t)k * P.N[1] + j) * P.N[0] + i];
   }
@@ -62,12 +67,14 @@ static void gather(const View& V, int i, int j, int k, bool all_d1, T* u, Derivs
   for (int f = 0; f < NF; ++f) u[f] = T(V.at(f, i, j, k));
   for (int f = 0; f < NF; ++f) {
     const bool o6 = sixth_order(V.P);
+    const int width = o6 ? 4 : 3;
     T line[3][9];
     for (int a = 0; a < 3; ++a)
       for (int s = -4; s <= 4; ++s) {
         int q[3] = {c[0], c[1], c[2]};
         q[a] += s;
-        line[a][s + 4] = T(V.at(f, q[0], q[1], q[2]));
+        // offsets beyond the stencil half-width are never used (and do not exist in a padded array)
+        line[a][s + 4] = (s < -width || s > width) ? T(0.0) : T(V.at(f, q[0], q[1], q[2]));
       }
     T adv = T(0.0), ko = T(0.0);
     for (int a = 0; a < 3; ++a) {
@@ -97,9 +104,9 @@ static void gather(const View& V, int i, int j, int k, bool all_d1, T* u, Derivs
 }
 
 // ---- S2+S3 over the grid: rhs = F(y) + Q_KO(y) ------------------------------------------
-static void rhs_global(const Params& P, const double* u, double* rhs) {
-  View V(P, u);
-  const size_t nc = V.ncell;
+static void rhs_global(const Params& P, const double* u, double* rhs, int pad = 0) {
+  View V(P, u, pad);
+  const size_t nc = (size_t)P.N[0] * P.N[1] * P.N[2];   // rhs holds interior cells only
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < P.N[2]; ++k)
     for (int j = 0; j < P.N[1]; ++j)
@@ -176,48 +183,168 @@ static int enforce_global(const Params& P, double* u, int do_enforce) {
 }
 
 // ---- O6 RK4, 3-register recurrence -------------------------------------------------------
-static int step_global(const Params& P, double* y, int nsteps, int do_enforce) {
-  const size_t n = (size_t)NF * P.N[0] * P.N[1] * P.N[2];
-  std::vector<double> Pr(n), Q(n), L(n);
-  const double dt = P.cfl * P.dx;
-  int bad = 0;
-  for (int st = 0; st < nsteps; ++st) {
+// One stage of the recurrence on n values: L = F(y) + Q_KO(y) of the current y. (One function so that the
+// single-level and the two-level drivers run the very same statements.)
+static void rk_stage_update(int stage, size_t n, double dt, const double* L, double* y, double* Pr, double* Q) {
+  if (stage == 1) {
     // stage 1: P = L(y); Q = P; y = E(y + P/2)
-    rhs_global(P, y, L.data());
 #pragma omp parallel for schedule(static)
     for (long long q = 0; q < (long long)n; ++q) {
       Pr[q] = dt * L[q];
       Q[q] = Pr[q];
       y[q] = y[q] + 0.5 * Pr[q];
     }
-    bad |= enforce_global(P, y, do_enforce);
+  } else if (stage == 2) {
     // stage 2: P = L(y); y = E(y + (P-Q)/2); Q = Q/6
-    rhs_global(P, y, L.data());
 #pragma omp parallel for schedule(static)
     for (long long q = 0; q < (long long)n; ++q) {
       Pr[q] = dt * L[q];
       y[q] = y[q] + 0.5 * (Pr[q] - Q[q]);
       Q[q] = Q[q] / 6.0;
     }
-    bad |= enforce_global(P, y, do_enforce);
+  } else if (stage == 3) {
     // stage 3: P = L(y) - P/2; y = E(y + P); Q = Q - P
-    rhs_global(P, y, L.data());
 #pragma omp parallel for schedule(static)
     for (long long q = 0; q < (long long)n; ++q) {
       Pr[q] = dt * L[q] - 0.5 * Pr[q];
       y[q] = y[q] + Pr[q];
       Q[q] = Q[q] - Pr[q];
     }
-    bad |= enforce_global(P, y, do_enforce);
+  } else {
     // stage 4: P = L(y) + 2P; y = E(y + (Q + P/6))
-    rhs_global(P, y, L.data());
 #pragma omp parallel for schedule(static)
     for (long long q = 0; q < (long long)n; ++q) {
       Pr[q] = dt * L[q] + 2.0 * Pr[q];
       y[q] = y[q] + (Q[q] + Pr[q] / 6.0);
     }
-    bad |= enforce_global(P, y, do_enforce);
   }
+}
+
+static int step_global(const Params& P, double* y, int nsteps, int do_enforce) {
+  const size_t n = (size_t)NF * P.N[0] * P.N[1] * P.N[2];
+  std::vector<double> Pr(n), Q(n), L(n);
+  const double dt = P.cfl * P.dx;
+  int bad = 0;
+  for (int st = 0; st < nsteps; ++st)
+    for (int stage = 1; stage <= 4; ++stage) {
+      rhs_global(P, y, L.data());
+      rk_stage_update(stage, n, dt, L.data(), y, Pr.data(), Q.data());
+      bad |= enforce_global(P, y, do_enforce);
+    }
+  return bad;
+}
+
+// ---- NEXT-3: restriction / prolongation at a factor-2 refinement boundary (z4c_amr.hpp) -----------
+// Restriction, step 1 of MeshBlock B's protocol ("Restrict the data in the active region to fill the
+// coarse buffer"). fine: [nfields][Nf_z][Nf_y][Nf_x], the active cells of the fine region in global fine order,
+// tiled by MeshBlocks of nf^3 cells; coarse: [nfields][Nf_z/2][Nf_y/2][Nf_x/2]. Eq. (2) with the outer product
+// of the three 1-D weight sets, summed z-outermost, x-innermost.
+static void restrict_region(int ng, int nf, const int32_t* Nf, const double* fine, double* coarse, int nfields) {
+  const int n = ng + 1;
+  const int Mc[3] = {Nf[0] / 2, Nf[1] / 2, Nf[2] / 2};
+  const size_t nfc = (size_t)Nf[0] * Nf[1] * Nf[2], ncc = (size_t)Mc[0] * Mc[1] * Mc[2];
+#pragma omp parallel for schedule(static)
+  for (int K = 0; K < Mc[2]; ++K)
+    for (int J = 0; J < Mc[1]; ++J)
+      for (int I = 0; I < Mc[0]; ++I) {
+        const int C[3] = {I, J, K};
+        double w[3][8];
+        int s[3];
+        for (int a = 0; a < 3; ++a) {
+          const int blk = (2 * C[a]) / nf;                 // the fine MeshBlock that owns the children
+          const int Il = C[a] - blk * (nf / 2);            // coarse index local to that block
+          s[a] = blk * nf + restrict_weights(Il, n, nf, w[a]);
+        }
+        for (int f = 0; f < nfields; ++f) {
+          double sum = 0.0;
+          for (int c = 0; c < n; ++c)
+            for (int b = 0; b < n; ++b)
+              for (int a = 0; a < n; ++a)
+                sum = sum + ((w[2][c] * w[1][b]) * w[0][a]) *
+                                fine[(size_t)f * nfc + ((size_t)(s[2] + c) * Nf[1] + (s[1] + b)) * Nf[0] + (s[0] + a)];
+          coarse[(size_t)f * ncc + ((size_t)K * Mc[1] + J) * Mc[0] + I] = sum;
+        }
+      }
+}
+
+// Prolongation, step 5 ("Prolongate the coarse buffer to fill the fine ghost zones"): the value at the
+// fine node (i, j, k) -- fine indices relative to the corner of the fine region, any sign -- from the coarse level
+// coarse[nfields][Nc_z][Nc_y][Nc_x] (global array, neighbours by wrap/clamp as in O2); the fine region's corner is
+// the coarse cell `origin`.
+static double prolong_point(int ng, const int32_t* Nc, int bc, const int32_t* origin, const double* coarse, int f,
+                            int i, int j, int k) {
+  const int n = ng + 1;
+  const int q[3] = {i, j, k};
+  double w[3][8];
+  int s[3];
+  for (int a = 0; a < 3; ++a) s[a] = origin[a] + prolong_weights(q[a], n, w[a]);
+  const size_t ncc = (size_t)Nc[0] * Nc[1] * Nc[2];
+  double sum = 0.0;
+  for (int c = 0; c < n; ++c)
+    for (int b = 0; b < n; ++b)
+      for (int a = 0; a < n; ++a) {
+        const int ii = map_index(s[0] + a, Nc[0], bc), jj = map_index(s[1] + b, Nc[1], bc),
+                  kk = map_index(s[2] + c, Nc[2], bc);
+        sum = sum + ((w[2][c] * w[1][b]) * w[0][a]) * coarse[(size_t)f * ncc + ((size_t)kk * Nc[1] + jj) * Nc[0] + ii];
+      }
+  return sum;
+}
+
+// Two-level state helpers: covered coarse cells <- restriction of the fine level; padded fine array <- fine
+// interior + ghost layers by prolongation (all faces, edges and corners of the fine region).
+static void two_level_sync(const Params& Pc, const Params& Pf, int nf, const int32_t* origin, double* uc,
+                           const double* uf, double* ufp) {
+  const int g = Pf.ng;
+  const int Mc[3] = {Pf.N[0] / 2, Pf.N[1] / 2, Pf.N[2] / 2};
+  std::vector<double> R((size_t)NF * Mc[0] * Mc[1] * Mc[2]);
+  restrict_region(g, nf, Pf.N, uf, R.data(), NF);
+  const size_t ncc = (size_t)Pc.N[0] * Pc.N[1] * Pc.N[2], nrc = (size_t)Mc[0] * Mc[1] * Mc[2];
+  for (int f = 0; f < NF; ++f)
+    for (int K = 0; K < Mc[2]; ++K)
+      for (int J = 0; J < Mc[1]; ++J)
+        for (int I = 0; I < Mc[0]; ++I)
+          uc[(size_t)f * ncc + ((size_t)(origin[2] + K) * Pc.N[1] + (origin[1] + J)) * Pc.N[0] + (origin[0] + I)] =
+              R[(size_t)f * nrc + ((size_t)K * Mc[1] + J) * Mc[0] + I];
+  const int mx = Pf.N[0] + 2 * g, my = Pf.N[1] + 2 * g, mz = Pf.N[2] + 2 * g;
+  const size_t npf = (size_t)mx * my * mz, nif = (size_t)Pf.N[0] * Pf.N[1] * Pf.N[2];
+#pragma omp parallel for schedule(static)
+  for (int k = -g; k < Pf.N[2] + g; ++k)
+    for (int j = -g; j < Pf.N[1] + g; ++j)
+      for (int i = -g; i < Pf.N[0] + g; ++i) {
+        const bool inside = i >= 0 && i < Pf.N[0] && j >= 0 && j < Pf.N[1] && k >= 0 && k < Pf.N[2];
+        for (int f = 0; f < NF; ++f)
+          ufp[(size_t)f * npf + ((size_t)(k + g) * my + (j + g)) * mx + (i + g)] =
+              inside ? uf[(size_t)f * nif + ((size_t)k * Pf.N[1] + j) * Pf.N[0] + i]
+                     : prolong_point(g, Pc.N, Pc.bc, origin, uc, f, i, j, k);
+      }
+}
+
+// Two-level static refinement (the set-up of the test at PAPER.md:171): the coarse level covers the
+// whole mesh, the fine level a box whose corner is the coarse cell `origin`; both advance with the same dt (no
+// subcycling), and after every RK stage the protocol of section 3.1 runs: restrict the fine active region into the
+// coarse nodes it covers (step B.1; those nodes are what the coarse neighbours receive, steps A.2 / B.2), then
+// prolongate the coarse level into the fine ghost zones (step B.5). Returns 1 if a bad cell was seen, -1 if the two
+// parameter sets do not describe one time step.
+static int step_two_level(const Params& Pc, const Params& Pf, int nf, const int32_t* origin, double* uc, double* uf,
+                          int nsteps) {
+  const double dt = Pc.cfl * Pc.dx;
+  if (std::fabs(dt - Pf.cfl * Pf.dx) > 1e-14 * dt || Pf.ng != Pc.ng) return -1;
+  const int g = Pf.ng;
+  const size_t ncn = (size_t)NF * Pc.N[0] * Pc.N[1] * Pc.N[2], nfn = (size_t)NF * Pf.N[0] * Pf.N[1] * Pf.N[2];
+  const size_t npf = (size_t)NF * (Pf.N[0] + 2 * g) * (Pf.N[1] + 2 * g) * (Pf.N[2] + 2 * g);
+  std::vector<double> Prc(ncn), Qc(ncn), Lc(ncn), Prf(nfn), Qf(nfn), Lf(nfn), ufp(npf);
+  int bad = 0;
+  two_level_sync(Pc, Pf, nf, origin, uc, uf, ufp.data());
+  for (int st = 0; st < nsteps; ++st)
+    for (int stage = 1; stage <= 4; ++stage) {
+      rhs_global(Pc, uc, Lc.data());
+      rhs_global(Pf, ufp.data(), Lf.data(), g);
+      rk_stage_update(stage, ncn, dt, Lc.data(), uc, Prc.data(), Qc.data());
+      bad |= enforce_global(Pc, uc, 1);
+      rk_stage_update(stage, nfn, dt, Lf.data(), uf, Prf.data(), Qf.data());
+      bad |= enforce_global(Pf, uf, 1);
+      two_level_sync(Pc, Pf, nf, origin, uc, uf, ufp.data());
+    }
   return bad;
 }
 
@@ -277,6 +404,30 @@ int oz4c_step(const Params* P, double* u, int nsteps, int do_enforce) {
 void oz4c_step_textbook(const Params* P, double* u, int nsteps) { step_textbook(*P, u, nsteps); }
 
 double oz4c_inv_cbrt(double x) { return inv_cbrt_spec(x); }
+
+// NEXT-3. Eq. (1) weights; restriction / prolongation stencil positions and weights along one
+// axis (readings Q21, Q22); the two operators on arrays; the two-level RK4 step.
+void oz4c_lagrange_weights(int n, const double* xs, double x, double* w) { lagrange_weights(n, xs, x, w); }
+int oz4c_restrict_weights(int Il, int ng, int nf, double* w) { return restrict_weights(Il, ng + 1, nf, w); }
+int oz4c_prolong_weights(int i, int ng, double* w) { return prolong_weights(i, ng + 1, w); }
+void oz4c_restrict(int ng, int nf, const int32_t* Nf, const double* fine, double* coarse, int nfields) {
+  restrict_region(ng, nf, Nf, fine, coarse, nfields);
+}
+// out[nfields][hi2-lo2][hi1-lo1][hi0-lo0]: prolonged values on the fine index box [lo, hi) (relative to the region)
+void oz4c_prolong(int ng, const int32_t* Nc, int bc, const int32_t* origin, const double* coarse, const int32_t* lo,
+                  const int32_t* hi, double* out, int nfields) {
+  const size_t nx = hi[0] - lo[0], ny = hi[1] - lo[1], nz = hi[2] - lo[2];
+  for (int f = 0; f < nfields; ++f)
+    for (int k = lo[2]; k < hi[2]; ++k)
+      for (int j = lo[1]; j < hi[1]; ++j)
+        for (int i = lo[0]; i < hi[0]; ++i)
+          out[(size_t)f * nx * ny * nz + ((size_t)(k - lo[2]) * ny + (j - lo[1])) * nx + (i - lo[0])] =
+              prolong_point(ng, Nc, bc, origin, coarse, f, i, j, k);
+}
+int oz4c_step_two_level(const Params* Pc, const Params* Pf, int nf, const int32_t* origin, double* uc, double* uf,
+                        int nsteps) {
+  return step_two_level(*Pc, *Pf, nf, origin, uc, uf, nsteps);
+}
 
 // S5: out = {H_rms,H_max,M_rms,M_max,Theta_rms,Theta_max,Z_rms,Z_max};
 // percell nullable: [4][Nz][Ny][Nx] = H, Mx, My, Mz

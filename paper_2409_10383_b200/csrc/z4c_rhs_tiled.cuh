@@ -448,7 +448,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
 //   8-wide tiles (8x4x4, 8x8x2: 20 % fewer halo bytes) are 20 % slower: 64-byte rows halve the coalescing of the
 //   register / state rows and put two tile rows of a warp on the same shared-memory banks.
-#if Z4C_NG == 3
+#if defined(Z4C_EXP_TZ)
+using RhsTile = TileCfg<16, 4, Z4C_EXP_TZ, Z4C_EXP_NSTAGE, Z4C_EXP_MINB>;   // tile experiments
+#elif Z4C_NG == 3
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
 #else
 // 4 ghosts: the halo tile grows to 24 x 12 x 10 (23 KB); to keep 2 CTAs per SM the P/Q tiles are read by batched
