@@ -117,6 +117,29 @@ int z4c_constraints(z4c_ctx* ctx, double* out, double* d_percell);
 int z4c_refine_indicators(z4c_ctx* ctx, double chi_min, double dchi_max, double* d_minchi, double* d_maxdchi,
                           int32_t* d_flags);
 
+/* --- NEXT-3: two-level static refinement (section 3.1) ------------------------------------------
+ * Two contexts on ONE stream: `coarse` covers the whole mesh, `fine` is a pack whose blocks tile a box of the coarse
+ * mesh at half the spacing (fine dx = coarse dx / 2, even n); origin[3] (host pointer) = global coarse cell index of
+ * the box's lower corner. The operators are Lagrange interpolation, Eq. (1)-(2) with n = N_g + 1
+ * nodes per axis and the outer product of the per-axis weights; all 22 fields are
+ * interpolated as they are (no re-enforcement of det gt = 1 / tr At = 0 on interpolated values).
+ *
+ * z4c_restrict: step 1 of MeshBlock B's protocol: every coarse interior cell covered by the fine box <-
+ *   interpolation of the fine ACTIVE cells; the stencil is the n nearest fine nodes, shifted so that it never leaves
+ *   the active region of the fine block that owns the cell's children. Then the coarse ghosts are
+ *   refilled, which hands the new values to the coarse neighbours (steps A.2 / B.2). Async.
+ * z4c_prolongate: step 5: every ghost cell of the fine pack that lies outside the fine box (faces, edges
+ *   and corners) <- interpolation of the n^3 nearest coarse nodes, read from the coarse INTERIOR cells through the
+ *   coarse level's own wrap / clamp rule. Fine ghosts inside the box are the same-level exchange's. Async.
+ * z4c_two_level_step: nsteps RK4 steps of both levels with one dt (no subcycling: coarse cfl*dx must equal fine
+ *   cfl*dx); after every stage: stage update with same-level ghost push on both packs, z4c_restrict, z4c_prolongate
+ *   (and once on entry, so the levels are consistent whatever the caller loaded). The set-up of the paper's
+ *   refined-corner wave test. Runs the unfused launch sequence (RHS, update + push per level). Async.
+ * Errors: Z4C_EINVAL (different streams, spacing not 2:1, box outside the coarse mesh, odd n, unequal dt). */
+int z4c_restrict(z4c_ctx* fine, z4c_ctx* coarse, const int32_t* origin);
+int z4c_prolongate(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin);
+int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, int nsteps);
+
 /* Inverse of z4c_set_initial_data: gather the interior cells of the pack into an interior
  * array. host pointer (on_device = 0; synchronises; staged through the workspace, so the RK
  * registers must not be live, i.e. not between stages -- always true between API calls) or

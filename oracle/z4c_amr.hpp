@@ -29,6 +29,14 @@
 //       even n because the fine node is off-centre by 1/4; centred on the parent cell for odd n).
 //   Q23 the 22 fields are interpolated as they are; the algebraic constraints are not re-imposed
 //       on interpolated values (the paper does not mention it).
+//   R-I1 floating-point form of Eq. (1)-(2). Because sum_i l_i = 1, Eq. (2) is evaluated as
+//       f(x) = f_r + sum_i l_i (f(x_i) - f_r), r = the stencil node nearest the target (the lower child for
+//       restriction, the parent node for prolongation): on a nearly flat background the differences are exact and
+//       the rounding error is relative to the perturbation, not to the O(1) field -- the same reason as the
+//       difference-from-centre stencils (Q14); an ulp of chi or gt_ii in a ghost node is otherwise amplified by
+//       dt/h^2 into At_ij. Eq. (1) is evaluated as one product of numerators over one product of denominators (all
+//       exact multiples of 1/4), so every weight is the exact dyadic rational. The 3-D weight is (l_z l_y) l_x and
+//       the sum runs z outermost, x innermost, every operation rounded separately: oracle and GPU agree bit for bit.
 // =====================================================================================
 #pragma once
 #include <cmath>
@@ -38,12 +46,13 @@ namespace oz4c {
 // Eq. (1): weights of the n nodes xs[0..n) at the point x.
 inline void lagrange_weights(int n, const double* xs, double x, double* w) {
   for (int i = 0; i < n; ++i) {
-    double l = 1.0;
+    double num = 1.0, den = 1.0;
     for (int m = 0; m < n; ++m) {
       if (m == i) continue;
-      l = l * ((x - xs[m]) / (xs[i] - xs[m]));
+      num = num * (x - xs[m]);
+      den = den * (xs[i] - xs[m]);
     }
-    w[i] = l;
+    w[i] = num / den;
   }
 }
 
@@ -66,6 +75,9 @@ inline int restrict_weights(int Il, int n, int nf, double* w) {
   return s;
 }
 
+// R-I1 reference node, as an index into the stencil: the lower child 2 Il (restriction), the parent I (prolongation)
+inline int restrict_ref(int Il, int n, int nf) { return 2 * Il - restrict_start(Il, n, nf); }
+
 // Q22: first coarse node of the prolongation stencil of fine node i (any sign), and its weights.
 inline int prolong_weights(int i, int n, double* w) {
   const int I = floor_div2(i);
@@ -77,6 +89,11 @@ inline int prolong_weights(int i, int n, double* w) {
   for (int q = 0; q < n; ++q) xs[q] = (double)(s + q);
   lagrange_weights(n, xs, (double)I - 0.25 + 0.5 * p, w);
   return s;
+}
+inline int prolong_ref(int i, int n) {
+  const int I = floor_div2(i);
+  const int p = i - 2 * I;
+  return (n % 2 == 0) ? n / 2 - p : (n - 1) / 2;
 }
 
 }  // namespace oz4c

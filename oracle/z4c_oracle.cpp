@@ -249,20 +249,23 @@ static void restrict_region(int ng, int nf, const int32_t* Nf, const double* fin
       for (int I = 0; I < Mc[0]; ++I) {
         const int C[3] = {I, J, K};
         double w[3][8];
-        int s[3];
+        int s[3], r[3];
         for (int a = 0; a < 3; ++a) {
           const int blk = (2 * C[a]) / nf;                 // the fine MeshBlock that owns the children
           const int Il = C[a] - blk * (nf / 2);            // coarse index local to that block
           s[a] = blk * nf + restrict_weights(Il, n, nf, w[a]);
+          r[a] = restrict_ref(Il, n, nf);
         }
         for (int f = 0; f < nfields; ++f) {
-          double sum = 0.0;
+          const double* F = fine + (size_t)f * nfc;
+          const double fr = F[((size_t)(s[2] + r[2]) * Nf[1] + (s[1] + r[1])) * Nf[0] + (s[0] + r[0])];
+          double sum = 0.0;                                // R-I1: f_r + sum W (f - f_r)
           for (int c = 0; c < n; ++c)
             for (int b = 0; b < n; ++b)
               for (int a = 0; a < n; ++a)
                 sum = sum + ((w[2][c] * w[1][b]) * w[0][a]) *
-                                fine[(size_t)f * nfc + ((size_t)(s[2] + c) * Nf[1] + (s[1] + b)) * Nf[0] + (s[0] + a)];
-          coarse[(size_t)f * ncc + ((size_t)K * Mc[1] + J) * Mc[0] + I] = sum;
+                                (F[((size_t)(s[2] + c) * Nf[1] + (s[1] + b)) * Nf[0] + (s[0] + a)] - fr);
+          coarse[(size_t)f * ncc + ((size_t)K * Mc[1] + J) * Mc[0] + I] = fr + sum;
         }
       }
 }
@@ -276,18 +279,23 @@ static double prolong_point(int ng, const int32_t* Nc, int bc, const int32_t* or
   const int n = ng + 1;
   const int q[3] = {i, j, k};
   double w[3][8];
-  int s[3];
-  for (int a = 0; a < 3; ++a) s[a] = origin[a] + prolong_weights(q[a], n, w[a]);
+  int s[3], r[3];
+  for (int a = 0; a < 3; ++a) {
+    s[a] = origin[a] + prolong_weights(q[a], n, w[a]);
+    r[a] = prolong_ref(q[a], n);
+  }
   const size_t ncc = (size_t)Nc[0] * Nc[1] * Nc[2];
-  double sum = 0.0;
+  auto at = [&](int a, int b, int c) {
+    const int ii = map_index(s[0] + a, Nc[0], bc), jj = map_index(s[1] + b, Nc[1], bc),
+              kk = map_index(s[2] + c, Nc[2], bc);
+    return coarse[(size_t)f * ncc + ((size_t)kk * Nc[1] + jj) * Nc[0] + ii];
+  };
+  const double fr = at(r[0], r[1], r[2]);
+  double sum = 0.0;                                        // R-I1: f_r + sum W (f - f_r)
   for (int c = 0; c < n; ++c)
     for (int b = 0; b < n; ++b)
-      for (int a = 0; a < n; ++a) {
-        const int ii = map_index(s[0] + a, Nc[0], bc), jj = map_index(s[1] + b, Nc[1], bc),
-                  kk = map_index(s[2] + c, Nc[2], bc);
-        sum = sum + ((w[2][c] * w[1][b]) * w[0][a]) * coarse[(size_t)f * ncc + ((size_t)kk * Nc[1] + jj) * Nc[0] + ii];
-      }
-  return sum;
+      for (int a = 0; a < n; ++a) sum = sum + ((w[2][c] * w[1][b]) * w[0][a]) * (at(a, b, c) - fr);
+  return fr + sum;
 }
 
 // Two-level state helpers: covered coarse cells <- restriction of the fine level; padded fine array <- fine

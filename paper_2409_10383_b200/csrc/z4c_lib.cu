@@ -10,6 +10,7 @@
 #include <string>
 
 #include "../../include/z4c.h"
+#include "z4c_amr.cuh"
 #include "z4c_kernels.cuh"
 #include "z4c_rhs_tiled.cuh"
 
@@ -497,6 +498,80 @@ int z4c_probe_fp64(void* cuda_stream, void* d_scratch, int iters, double* tflops
   if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return Z4C_ECUDA;
   *tflops_out = 2.0 * 8.0 * (double)iters * (double)grid * threads / ((double)ms * 1e-3) * 1e-12;
   return Z4C_OK;
+}
+
+// ---- NEXT-3: two-level static refinement ------------------------------------------------
+namespace {
+// The fine pack must be the factor-2 refinement of a box of the coarse pack, both on one stream with one dt.
+int check_levels(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, AmrGeom* a) {
+  if (!coarse || !fine || !origin || coarse == fine) return Z4C_EINVAL;
+  if (coarse->stream != fine->stream) return fail(fine, Z4C_EINVAL, "two-level calls need both contexts on one stream");
+  if (fine->g.n % 2) return fail(fine, Z4C_EINVAL, "restriction needs an even block size");
+  if (std::fabs(2.0 * fine->prm.dx - coarse->prm.dx) > 1e-12 * coarse->prm.dx)
+    return fail(fine, Z4C_EINVAL, "fine dx must be half the coarse dx");
+  for (int d = 0; d < 3; ++d) {
+    a->origin[d] = origin[d];
+    a->Mc[d] = fine->g.n * fine->g.nb[d] / 2;
+    if (origin[d] < 0 || origin[d] + a->Mc[d] > coarse->g.n * coarse->g.nb[d])
+      return fail(fine, Z4C_EINVAL, "fine region does not lie inside the coarse mesh");
+  }
+  return Z4C_OK;
+}
+int launch_restrict(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a) {
+  const long long total = (long long)a.Mc[0] * a.Mc[1] * a.Mc[2] * NF;
+  k_restrict<<<grid_for(total, 128), 128, 0, fine->stream>>>(fine->g, fine->y, coarse->g, coarse->y, a);
+  return check_launch(fine, "k_restrict");
+}
+int launch_prolong(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a) {
+  const Pack& g = fine->g;
+  const long long per_block = 2LL * NG * ((long long)g.m * g.m + (long long)g.n * g.m + (long long)g.n * g.n);
+  k_prolong<<<grid_for(per_block * g.nblk * NF, 128), 128, 0, fine->stream>>>(coarse->g, coarse->y, g, fine->y, a);
+  return check_launch(fine, "k_prolong");
+}
+// steps B.1, A.2/B.2 (the covered coarse nodes reach the coarse neighbours through the same-level fill), B.5
+int sync_levels(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a) {
+  int rc = launch_restrict(coarse, fine, a);
+  if (rc) return rc;
+  rc = launch_ghost_fill(coarse);
+  if (rc) return rc;
+  return launch_prolong(coarse, fine, a);
+}
+}  // namespace
+
+int z4c_restrict(z4c_ctx* fine, z4c_ctx* coarse, const int32_t* origin) {
+  AmrGeom a;
+  int rc = check_levels(coarse, fine, origin, &a);
+  if (rc) return rc;
+  rc = launch_restrict(coarse, fine, a);
+  if (rc) return rc;
+  return launch_ghost_fill(coarse);
+}
+
+int z4c_prolongate(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin) {
+  AmrGeom a;
+  int rc = check_levels(coarse, fine, origin, &a);
+  if (rc) return rc;
+  return launch_prolong(coarse, fine, a);
+}
+
+int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, int nsteps) {
+  static const double coef[4] = {0.0, 0.0, -0.5, 2.0};
+  AmrGeom a;
+  int rc = check_levels(coarse, fine, origin, &a);
+  if (rc) return rc;
+  if (nsteps < 0) return Z4C_EINVAL;
+  if (std::fabs(coarse->dt - fine->dt) > 1e-14 * fine->dt)
+    return fail(fine, Z4C_EINVAL, "both levels advance with one dt (no subcycling): set cfl so that cfl*dx agrees");
+  rc = sync_levels(coarse, fine, a);
+  for (int st = 0; st < nsteps && rc == Z4C_OK; ++st)
+    for (int s = 1; s <= 4 && rc == Z4C_OK; ++s) {
+      z4c_ctx* lv[2] = {coarse, fine};
+      for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_rhs(lv[q], coef[s - 1], lv[q]->dt);
+      for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_stage_update(lv[q], s, true);
+      if (rc == Z4C_OK) rc = sync_levels(coarse, fine, a);
+    }
+  if (rc == Z4C_OK) { coarse->steps += nsteps; fine->steps += nsteps; }
+  return rc;
 }
 
 int z4c_sync(z4c_ctx* c) {

@@ -23,6 +23,7 @@ SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_init
            "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
            "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
            "z4c_probe_fp64", "z4c_effective_mode", "z4c_time",
+           "z4c_restrict", "z4c_prolongate", "z4c_two_level_step",
            "z4c_last_error", "z4c_destroy"]
 
 
@@ -87,6 +88,10 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.z4c_probe_fp64.argtypes = [vp, vp, C.c_int, C.POINTER(C.c_double)]
     L.z4c_effective_mode.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    i3 = C.POINTER(C.c_int32)
+    L.z4c_restrict.argtypes = [vp, vp, i3]
+    L.z4c_prolongate.argtypes = [vp, vp, i3]
+    L.z4c_two_level_step.argtypes = [vp, vp, i3, C.c_int]
     L.z4c_time.argtypes = [vp]
     L.z4c_time.restype = C.c_double
     L.z4c_last_error.argtypes = [vp]
@@ -95,7 +100,8 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_destroy.restype = None
     for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior",
                "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
-               "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64", "z4c_effective_mode"):
+               "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64", "z4c_effective_mode", "z4c_restrict", "z4c_prolongate",
+               "z4c_two_level_step"):
         getattr(L, fn).restype = C.c_int
     if path == default:
         _libs[ng] = L
@@ -281,6 +287,25 @@ class Z4c:
         if rc != 0:
             raise Z4cError(rc, "z4c_probe_fp64 failed")
         return float(out.value)
+
+    # -- NEXT-3: two-level static refinement; `self` is the FINE level, `coarse` another Z4c on the same stream --
+    def restrict_to(self, coarse: "Z4c", origin):
+        """z4c_restrict(fine = self, coarse, origin)."""
+        o = (C.c_int32 * 3)(*[int(v) for v in origin])
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_restrict(self.h, coarse.h, o))
+
+    def prolongate_from(self, coarse: "Z4c", origin):
+        """z4c_prolongate(coarse, fine = self, origin)."""
+        o = (C.c_int32 * 3)(*[int(v) for v in origin])
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_prolongate(coarse.h, self.h, o))
+
+    def two_level_step(self, coarse: "Z4c", origin, nsteps: int = 1):
+        """z4c_two_level_step(coarse, fine = self, origin, nsteps)."""
+        o = (C.c_int32 * 3)(*[int(v) for v in origin])
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_two_level_step(coarse.h, self.h, o, int(nsteps)))
 
     def time(self) -> float:
         return float(self.lib.z4c_time(self.h))

@@ -31,7 +31,7 @@ def test_A1_weights_against_exact_rationals(oracle, ng):
         s, w = oracle.restrict_weights(Il, ng, nf)
         assert 0 <= s and s + n <= nf                                   # inside the active region
         ex = lagrange_exact(range(s, s + n), Fraction(4 * Il + 1, 2))    # the coarse node sits at 2 Il + 1/2
-        assert np.allclose(w, [float(e) for e in ex], rtol=0, atol=4e-16)
+        assert np.array_equal(w, [float(e) for e in ex])                # exact dyadic rationals (R-I1)
         assert sum(ex) == 1
         # Q21: unless a block face forces a shift, the stencil holds the n nodes nearest to the target
         free = 2 * Il + 1 - (n + 1) // 2
@@ -44,7 +44,7 @@ def test_A1_weights_against_exact_rationals(oracle, ng):
         s, w = oracle.prolong_weights(i, ng)
         X = Fraction(2 * i + 1, 4) - Fraction(1, 2)                     # fine node i in coarse-index units
         ex = lagrange_exact(range(s, s + n), X)
-        assert np.allclose(w, [float(e) for e in ex], rtol=0, atol=4e-16)
+        assert np.array_equal(w, [float(e) for e in ex])                # exact dyadic rationals (R-I1)
         d_in = max(abs(q - float(X)) for q in range(s, s + n))         # Q22: the n nearest coarse nodes
         d_out = min(abs(q - float(X)) for q in (s - 1, s + n))
         assert d_in <= d_out
@@ -204,3 +204,22 @@ def test_A7_two_level_rejects_mismatched_time_steps(oracle):
     pc, pf = _two_level_wave(32, 16)
     bad = oracle.step_two_level(replace(pc, cfl=0.25), pf, 16, (0, 0, 0), I.minkowski(pc), I.minkowski(pf), 1)[2]
     assert bad == -1
+
+
+def test_A8_difference_from_reference_form_reproduces_constants_bitwise(oracle):
+    """R-I1: Eq. (2) as f_r + sum l_i (f_i - f_r). A constant that is not a dyadic rational comes back bit for bit from
+    both operators (a plain weighted sum would round 64 products), and a 1e-8 perturbation of 1 is interpolated with an
+    error far below one ulp of 1 before the final rounding."""
+    ng, nf = 3, 8
+    c = 0.1
+    fine = np.full((1, 16, 16, 16), c)
+    assert np.all(oracle.restrict(fine, ng, nf) == c)
+    coarse = np.full((1, 12, 12, 12), c)
+    assert np.all(oracle.prolong(coarse, ng, 0, (2, 2, 2), (-3, -3, -3), (11, 11, 11)) == c)
+    h = 1.0 / 16
+    xf = (np.arange(16) + 0.5) * h
+    xc = (np.arange(8) + 0.5) * 2 * h
+    pert = lambda z, y, x: 1e-8 * (x * x * y - z ** 3)
+    fine = (1.0 + pert(xf[:, None, None], xf[None, :, None], xf[None, None, :]))[None]
+    want = 1.0 + pert(xc[:, None, None], xc[None, :, None], xc[None, None, :])
+    assert np.abs(oracle.restrict(fine, ng, nf)[0] - want).max() <= 2.3e-16      # one final rounding of ~1
