@@ -140,6 +140,40 @@ int z4c_restrict(z4c_ctx* fine, z4c_ctx* coarse, const int32_t* origin);
 int z4c_prolongate(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin);
 int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, int nsteps);
 
+/* --- NEXT-2: one mesh partitioned over several packs / GPUs (the exchange: "at each
+ * stage ... the ghost zones are filled by ... the active region of neighboring MeshBlocks", 75-76 "Pack and send") ----
+ * The block lattice nb[0] x nb[1] x nbz_global of the whole mesh is cut into slabs along z; a context created with
+ * nb[2] = the slab's thickness owns the blocks bz0 <= bz < bz0 + nb[2] (one process and one GPU per slab). There is no
+ * pack / send / receive / unpack: the kernel that updates a cell writes that cell's ghost images straight into the
+ * pack that holds them, its own or a z-neighbour's (peer memory over NVLink, mapped into this process by the caller,
+ * e.g. through CUDA IPC), addressing three packs through one table. What remains of the exchange is a barrier between
+ * stages, which is the caller's (a stream-ordered collective of torch.distributed; see partition.py).
+ *
+ * z4c_set_partition: declare the slab. bc and wrap / clamp then refer to the whole lattice. Switches mode 0 to 1.
+ * z4c_set_neighbor: side 0 = the slab below (towards bz = 0; the top slab if periodic), 1 = the slab above.
+ *   d_state, d_state2: DEVICE pointers, valid in this process, of that slab's state buffer and second state buffer
+ *   (z4c_state2 of its context); bz0, nbz: its z-range. NULL, NULL = none on that side (outflow boundary). A slab
+ *   may be its own neighbour (one slab, periodic) -- then no call is needed: entry 0 of the table covers it.
+ * z4c_state2: device pointer of the context's second state buffer (lives in the workspace), to hand to neighbours.
+ * z4c_stage: ONE Runge-Kutta stage (1..4) in the context's fuse mode, asynchronous. Between two stages every slab
+ *   must have finished the previous one (barrier): stage s+1 reads ghosts its neighbours wrote in stage s, and writes
+ *   ghosts into the buffer they read in stage s. Stage 4 advances the context's time. z4c_step refuses a slab.
+ *   z4c_stage needs the one-kernel-per-stage mode (2), whose two state buffers make one barrier per stage enough. Where
+ *   that mode is unavailable (odd n, variant 1) the state is updated in place and a stage is two calls with a barrier
+ *   after each: z4c_stage_rhs (K2 into the RK register P), z4c_stage_update (K3 with ghost push; stage 4 advances time).
+ * z4c_set_initial_data on a slab loads and enforces the slab's interior only; after a barrier every slab calls
+ *   z4c_fill_ghosts (which pulls across slab faces), then another barrier.
+ * z4c_constraints_raw: like z4c_constraints but the four sums of squares are NOT divided and rooted:
+ *   out = {sum H^2, max|H|, sum |M|^2, max|M|, sum Theta^2, max|Theta|, sum |Z|^2, max|Z|} over this slab, so that the
+ *   mesh-wide norms are one 8-double all-reduce away (SUM on even, MAX on odd entries). Synchronises the stream. */
+int z4c_set_partition(z4c_ctx* ctx, int32_t nbz_global, int32_t bz0);
+int z4c_set_neighbor(z4c_ctx* ctx, int32_t side, void* d_state, void* d_state2, int32_t bz0, int32_t nbz);
+void* z4c_state2(const z4c_ctx* ctx);
+int z4c_stage(z4c_ctx* ctx, int stage);
+int z4c_stage_rhs(z4c_ctx* ctx, int stage);
+int z4c_stage_update(z4c_ctx* ctx, int stage);
+int z4c_constraints_raw(z4c_ctx* ctx, double* out);
+
 /* Inverse of z4c_set_initial_data: gather the interior cells of the pack into an interior
  * array. host pointer (on_device = 0; synchronises; staged through the workspace, so the RK
  * registers must not be live, i.e. not between stages -- always true between API calls) or

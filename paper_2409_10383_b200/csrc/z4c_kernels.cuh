@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(256) k_layout(Pack g, double* __restrict__ pac
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int ghost_coord(int q, int n) { return q < NG ? q : n + q; }  // q in [0, 2 NG)
 
-__global__ void __launch_bounds__(256) k_ghost_fill(Pack g, double* __restrict__ y) {
+__global__ void __launch_bounds__(256) k_ghost_fill(Pack g, double* __restrict__ y, Slab sl) {
   const int n = g.n, m = g.m;
   constexpr int G2 = 2 * NG;
   const int nZ = G2 * m * m, nY = G2 * n * m, nX = G2 * n * n;
@@ -69,13 +69,16 @@ __global__ void __launch_bounds__(256) k_ghost_fill(Pack g, double* __restrict__
     int sbx, sby, sbz, si, sj, sk;
     ghost_source(i, bx, n, g.nb[0], g.bc, sbx, si);
     ghost_source(j, by, n, g.nb[1], g.bc, sby, sj);
-    ghost_source(k, bz, n, g.nb[2], g.bc, sbz, sk);
-    const long long sb = ((long long)sbz * g.nb[1] + sby) * g.nb[0] + sbx;
+    ghost_source(k, sl.bz0[0] + bz, n, sl.nbz_global, g.bc, sbz, sk);   // z in the lattice of the whole mesh
+    const int e = slab_entry(sl, sbz);                                   // the pack that holds the source block
+    const long long sb = ((long long)(sbz - slab_bz0(sl, e)) * g.nb[1] + sby) * g.nb[0] + sbx;
     const long long src = sb * g.m3 + ((long long)sk * m + sj) * m + si;
     const long long dst = (long long)b * g.m3 + ((long long)k * m + j) * m + i;
+    const double* ys = slab_y(sl, e);
+    const long long sfs = slab_fs(sl, e);
     double v[NF];
 #pragma unroll
-    for (int f = 0; f < NF; ++f) v[f] = y[f * g.fs + src];
+    for (int f = 0; f < NF; ++f) v[f] = ys[f * sfs + src];
 #pragma unroll
     for (int f = 0; f < NF; ++f) y[f * g.fs + dst] = v[f];
   }
@@ -236,7 +239,7 @@ __device__ __forceinline__ int push_targets(int l, int bcoord, int n, int nbl, i
 template <int STAGE, bool PUSH>
 __global__ void __launch_bounds__(128) k_stage_update(Pack g, double* __restrict__ y, const double* __restrict__ Preg,
                                                       double* __restrict__ Qreg, double chi_floor,
-                                                      int* __restrict__ flag) {
+                                                      int* __restrict__ flag, Slab sl) {
   const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (t >= g.ncell) return;
   const int b = (int)(t / g.n3);
@@ -282,16 +285,20 @@ __global__ void __launch_bounds__(128) k_stage_update(Pack g, double* __restrict
       int tbx[NG + 1], tlx[NG + 1], tby[NG + 1], tly[NG + 1], tbz[NG + 1], tlz[NG + 1];
       const int cx = push_targets(i, bx, g.n, g.nb[0], g.bc, tbx, tlx);
       const int cy = push_targets(j, by, g.n, g.nb[1], g.bc, tby, tly);
-      const int cz = push_targets(k, bz, g.n, g.nb[2], g.bc, tbz, tlz);
-      for (int a = 0; a < cz; ++a)
+      const int cz = push_targets(k, sl.bz0[0] + bz, g.n, sl.nbz_global, g.bc, tbz, tlz);   // global z lattice
+      for (int a = 0; a < cz; ++a) {
+        const int e = slab_entry(sl, tbz[a]);                      // the pack that holds the target block (NEXT-2)
+        double* ye = slab_y(sl, e);
+        const long long efs = slab_fs(sl, e);
         for (int bb = 0; bb < cy; ++bb)
           for (int cc = 0; cc < cx; ++cc) {
             if (a + bb + cc == 0) continue;  // the cell itself, already written
-            const long long tb = ((long long)tbz[a] * g.nb[1] + tby[bb]) * g.nb[0] + tbx[cc];
-            double* d = y + tb * g.m3 + ((long long)tlz[a] * g.m + tly[bb]) * g.m + tlx[cc];
+            const long long tb = ((long long)(tbz[a] - slab_bz0(sl, e)) * g.nb[1] + tby[bb]) * g.nb[0] + tbx[cc];
+            double* d = ye + tb * g.m3 + ((long long)tlz[a] * g.m + tly[bb]) * g.m + tlx[cc];
 #pragma unroll
-            for (int f = 0; f < NF; ++f) d[f * g.fs] = u[f];
+            for (int f = 0; f < NF; ++f) d[f * efs] = u[f];
           }
+      }
     }
   }
 }
@@ -404,7 +411,8 @@ __global__ void __launch_bounds__(KR_THREADS)
   }
 }
 
-// second pass: one CTA, fixed order. out[8] = {H_rms,H_max,M_rms,M_max,Theta_rms,Theta_max,Z_rms,Z_max}
+// second pass: one CTA, fixed order. out[8] = {H_rms,H_max,M_rms,M_max,Theta_rms,Theta_max,Z_rms,Z_max};
+// ncell < 0: the sums of squares are left as they are (a slab's share of a partitioned mesh, NEXT-2)
 __global__ void __launch_bounds__(K4_THREADS)
     k_constraints_final(const double* __restrict__ partial, int nparts, double ncell, double* __restrict__ out) {
   __shared__ double red[8 * (K4_THREADS / 32)];
@@ -419,7 +427,7 @@ __global__ void __launch_bounds__(K4_THREADS)
   block_reduce8(acc, red);
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int q = 0; q < 8; ++q) out[q] = (q & 1) ? acc[q] : sqrt(acc[q] / ncell);
+    for (int q = 0; q < 8; ++q) out[q] = (q & 1) || ncell < 0.0 ? acc[q] : sqrt(acc[q] / ncell);
   }
 }
 

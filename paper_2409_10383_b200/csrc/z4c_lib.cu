@@ -41,6 +41,10 @@ struct z4c_ctx {
   int num_sms;
   RegMaps rmap;         // TMA descriptors of the RK registers P, Q
   int have_ymap;
+  // NEXT-2: this pack is the slab [bz0, bz0 + nb[2]) of a lattice with nbz_global blocks along z
+  int bz0, nbz_global;
+  double* nbr_y[2][2];   // [lower, upper][state buffer 0, 1] of the neighbouring slabs (peer memory), or null
+  int nbr_bz0[2], nbr_nbz[2];
   std::string err;
 };
 
@@ -79,6 +83,23 @@ Pack make_pack(const z4c_params& p) {
   return g;
 }
 
+bool partitioned(const z4c_ctx* c) { return c->nbz_global != c->g.nb[2]; }
+
+// The table the ghost-writing (or -reading) kernels address: this pack's buffer `buf` and the same buffer of the two
+// z-neighbours (NEXT-2). Unpartitioned: one entry.
+Slab make_slab(const z4c_ctx* c, int buf) {
+  Slab s;
+  s.y[0] = c->ybuf[buf]; s.fs[0] = c->g.fs; s.bz0[0] = c->bz0; s.nbz[0] = c->g.nb[2];
+  for (int side = 0; side < 2; ++side) {
+    s.y[1 + side] = c->nbr_y[side][buf];
+    s.bz0[1 + side] = c->nbr_bz0[side];
+    s.nbz[1 + side] = c->nbr_y[side][buf] ? c->nbr_nbz[side] : 0;
+    s.fs[1 + side] = (long long)c->g.nb[0] * c->g.nb[1] * c->nbr_nbz[side] * c->g.m3;
+  }
+  s.nbz_global = c->nbz_global;
+  return s;
+}
+
 int fail(z4c_ctx* c, int code, const std::string& msg) {
   if (c) c->err = msg;
   return code;
@@ -102,14 +123,14 @@ int grid_for(long long total, int threads, long long cap = (1LL << 30)) {
 // ---- launch helpers (all asynchronous on c->stream) ---------------------------------------
 int launch_ghost_fill(z4c_ctx* c) {
   const long long per_block = 2LL * NG * ((long long)c->g.m * c->g.m + (long long)c->g.n * c->g.m + (long long)c->g.n * c->g.n);
-  k_ghost_fill<<<grid_for(per_block * c->g.nblk, 256), 256, 0, c->stream>>>(c->g, c->y);
+  k_ghost_fill<<<grid_for(per_block * c->g.nblk, 256), 256, 0, c->stream>>>(c->g, c->y, make_slab(c, 0));
   return check_launch(c, "k_ghost_fill");
 }
 
 int launch_rhs(z4c_ctx* c, double coef, double dt) {
   const Pack& g = c->g;
   if (c->variant != 1 && c->have_ymap) {
-    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], c->rmap, g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{c->y, nullptr, nullptr, 0.0, nullptr});
+    cudaError_t e = launch_rhs_tiled_t<RhsTile, 0>(c->ymap[0], c->rmap, g, c->P, c->fd, c->sp, coef, dt, c->stream, StageArgs{c->y, nullptr, Slab{}, 0.0, nullptr});
     if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
     return check_launch(c, "k_rhs_tiled");
   }
@@ -124,12 +145,13 @@ int launch_rhs(z4c_ctx* c, double coef, double dt) {
 template <bool PUSH>
 void launch_stage_update_t(z4c_ctx* c, int stage, int grid) {
   const Pack& g = c->g;
+  const Slab sl = make_slab(c, 0);
   switch (stage) {
-    case 0: k_stage_update<0, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
-    case 1: k_stage_update<1, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
-    case 2: k_stage_update<2, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
-    case 3: k_stage_update<3, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
-    default: k_stage_update<4, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag); break;
+    case 0: k_stage_update<0, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag, sl); break;
+    case 1: k_stage_update<1, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag, sl); break;
+    case 2: k_stage_update<2, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag, sl); break;
+    case 3: k_stage_update<3, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag, sl); break;
+    default: k_stage_update<4, PUSH><<<grid, 128, 0, c->stream>>>(g, c->y, c->P, c->Q, c->prm.chi_floor, c->flag, sl); break;
   }
 }
 
@@ -154,7 +176,7 @@ cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, const RegMa
   }
 }
 int launch_fused_stage(z4c_ctx* c, int stage, int in) {
-  StageArgs sa{c->ybuf[in], c->Q, c->ybuf[1 - in], c->prm.chi_floor, c->flag};
+  StageArgs sa{c->ybuf[in], c->Q, make_slab(c, 1 - in), c->prm.chi_floor, c->flag};
   cudaError_t e = launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
   return check_launch(c, "k_rhs_tiled<stage>");
@@ -317,6 +339,12 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->fuse_ghosts = 2;
   c->graph_exec = nullptr;
   c->graph_launches = 0;
+  c->bz0 = 0;
+  c->nbz_global = c->g.nb[2];
+  for (int side = 0; side < 2; ++side) {
+    c->nbr_y[side][0] = c->nbr_y[side][1] = nullptr;
+    c->nbr_bz0[side] = c->nbr_nbz[side] = 0;
+  }
   {
     int dev = 0;
     c->num_sms = 148;
@@ -360,8 +388,10 @@ int z4c_set_initial_data(z4c_ctx* c, const double* interior, int on_device) {
   if (rc) return rc;
   rc = launch_stage_update(c, 0, false);
   if (rc) return rc;
-  rc = launch_ghost_fill(c);
-  if (rc) return rc;
+  if (!partitioned(c)) {   // a slab's ghosts need its neighbours' data: z4c_fill_ghosts after a barrier (NEXT-2)
+    rc = launch_ghost_fill(c);
+    if (rc) return rc;
+  }
   const size_t reg = align_up((size_t)NF * (size_t)c->g.is * sizeof(double));
   rc = check_cuda(c, cudaMemsetAsync(c->P, 0, 2 * reg, c->stream), "memset registers");
   if (rc) return rc;
@@ -372,6 +402,8 @@ int z4c_set_initial_data(z4c_ctx* c, const double* interior, int on_device) {
 
 int z4c_step(z4c_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return Z4C_EINVAL;
+  if (partitioned(c))
+    return fail(c, Z4C_EINVAL, "a slab of a partitioned mesh advances stage by stage: z4c_stage + a barrier between stages");
   if (c->use_graph) {
     if (!c->graph_exec) {
       cudaGraph_t graph = nullptr;
@@ -574,6 +606,76 @@ int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, in
   return rc;
 }
 
+// ---- NEXT-2: partitioned mesh (ghost exchange at every stage) -----------
+int z4c_set_partition(z4c_ctx* c, int32_t nbz_global, int32_t bz0) {
+  if (!c) return Z4C_EINVAL;
+  if (bz0 < 0 || nbz_global < 1 || bz0 + c->g.nb[2] > nbz_global || nbz_global > (1 << 24)) return Z4C_EINVAL;
+  drop_graph(c);
+  c->nbz_global = nbz_global;
+  c->bz0 = bz0;
+  if (partitioned(c) && c->fuse_ghosts == 0) c->fuse_ghosts = 1;
+  return Z4C_OK;
+}
+
+int z4c_set_neighbor(z4c_ctx* c, int32_t side, void* d_state, void* d_state2, int32_t bz0, int32_t nbz) {
+  if (!c || side < 0 || side > 1) return Z4C_EINVAL;
+  if ((d_state || d_state2) && (!d_state || !d_state2 || nbz < 1 || bz0 < 0 || bz0 + nbz > c->nbz_global)) return Z4C_EINVAL;
+  drop_graph(c);
+  c->nbr_y[side][0] = (double*)d_state;
+  c->nbr_y[side][1] = (double*)d_state2;
+  c->nbr_bz0[side] = bz0;
+  c->nbr_nbz[side] = nbz;
+  return Z4C_OK;
+}
+
+void* z4c_state2(const z4c_ctx* c) { return c ? (void*)c->ybuf[1] : nullptr; }
+
+int z4c_stage(z4c_ctx* c, int stage) {
+  static const double coef[4] = {0.0, 0.0, -0.5, 2.0};
+  if (!c || stage < 1 || stage > 4) return Z4C_EINVAL;
+  int rc;
+  if (fully_fused(c)) {
+    rc = launch_fused_stage(c, stage, (stage - 1) & 1);
+  } else {
+    if (partitioned(c))
+      return fail(c, Z4C_EINVAL, "in modes 0/1 the state is updated in place: a slab needs a barrier between the RHS "
+                                 "and the update of a stage (z4c_stage_rhs, barrier, z4c_stage_update, barrier)");
+    rc = launch_rhs(c, coef[stage - 1], c->dt);
+    if (rc == Z4C_OK) rc = launch_stage_update(c, stage, c->fuse_ghosts != 0);
+    if (rc == Z4C_OK && !c->fuse_ghosts) rc = launch_ghost_fill(c);
+  }
+  if (rc == Z4C_OK && stage == 4) c->steps += 1;
+  return rc;
+}
+
+int z4c_stage_rhs(z4c_ctx* c, int stage) {
+  static const double coef[4] = {0.0, 0.0, -0.5, 2.0};
+  if (!c || stage < 1 || stage > 4) return Z4C_EINVAL;
+  return launch_rhs(c, coef[stage - 1], c->dt);
+}
+
+int z4c_stage_update(z4c_ctx* c, int stage) {
+  if (!c || stage < 1 || stage > 4) return Z4C_EINVAL;
+  int rc = launch_stage_update(c, stage, true);
+  if (rc == Z4C_OK && stage == 4) c->steps += 1;
+  return rc;
+}
+
+int z4c_constraints_raw(z4c_ctx* c, double* out) {
+  if (!c || !out) return Z4C_EINVAL;
+  int nparts = grid_for(c->g.ncell, K4_THREADS, K4_MAX_PARTS);
+  k_constraints<<<nparts, K4_THREADS, 0, c->stream>>>(c->g, c->y, c->fd, c->sp, c->partial, nullptr);
+  int rc = check_launch(c, "k_constraints");
+  if (rc) return rc;
+  k_constraints_final<<<1, K4_THREADS, 0, c->stream>>>(c->partial, nparts, -1.0, c->result);
+  rc = check_launch(c, "k_constraints_final");
+  if (rc) return rc;
+  rc = check_cuda(c, cudaMemcpyAsync(out, c->result, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream),
+                  "D2H copy");
+  if (rc) return rc;
+  return read_flag(c);
+}
+
 int z4c_sync(z4c_ctx* c) {
   if (!c) return Z4C_EINVAL;
   return read_flag(c);
@@ -598,6 +700,8 @@ int z4c_use_graph(z4c_ctx* c, int enable) {
 int z4c_set_fused(z4c_ctx* c, int enable) {
   if (!c) return Z4C_EINVAL;
   if (enable < 0 || enable > 2) return Z4C_EINVAL;
+  if (enable == 0 && partitioned(c))
+    return fail(c, Z4C_EINVAL, "a slab of a partitioned mesh pushes its ghost images (modes 1, 2): mode 0 would pull mid-stage");
   if (enable != c->fuse_ghosts) drop_graph(c);
   c->fuse_ghosts = enable;
   return Z4C_OK;

@@ -44,4 +44,26 @@ __host__ __device__ inline void ghost_source(int l, int bcoord, int n, int nbl, 
   sl = G - sb * n + NG;
 }
 
+// NEXT-2 (the exchange itself at PAPER.md:65, 75-76): the block lattice of the whole mesh is cut
+// into slabs along z, one MeshBlockPack (one process, one GPU) per slab. A cell's ghost images then live either in
+// this pack or in the pack of the slab below / above; the kernels that write (or read) ghost cells address the three
+// packs through this table. Entry 0 is the pack itself; entries 1 / 2 are the lower / upper neighbour, whose buffers
+// are mapped into this process (peer memory over NVLink). An unpartitioned pack is the one-entry case.
+struct Slab {
+  double* y[3];       // state buffer of each entry (the buffer being written -- or read, for the pull kernel)
+  long long fs[3];    // field stride of each entry's pack
+  int bz0[3], nbz[3]; // global z-range of the blocks of each entry (nbz = 0: absent)
+  int nbz_global;     // blocks along z of the whole lattice
+};
+// which entry owns the global block coordinate bz (after wrap / clamp in the global lattice)
+__host__ __device__ inline int slab_entry(const Slab& s, int bz) {
+  if (bz >= s.bz0[0] && bz < s.bz0[0] + s.nbz[0]) return 0;
+  if (bz >= s.bz0[1] && bz < s.bz0[1] + s.nbz[1]) return 1;
+  return 2;
+}
+// entry lookups by selects: a run-time index into a kernel-parameter array would send the table to local memory
+__host__ __device__ inline double* slab_y(const Slab& s, int e) { return e == 0 ? s.y[0] : (e == 1 ? s.y[1] : s.y[2]); }
+__host__ __device__ inline long long slab_fs(const Slab& s, int e) { return e == 0 ? s.fs[0] : (e == 1 ? s.fs[1] : s.fs[2]); }
+__host__ __device__ inline int slab_bz0(const Slab& s, int e) { return e == 0 ? s.bz0[0] : (e == 1 ? s.bz0[1] : s.bz0[2]); }
+
 }  // namespace z4c

@@ -221,7 +221,8 @@ struct FieldLoop<Cfg, FULL, NF> {
 struct StageArgs {
   const double* y_in;   // the state buffer the tensor map describes (centre values of gt_ij are read up front)
   double* Q;
-  double* y_out;
+  Slab out;             // where the new state goes: this pack's other buffer and, for a partitioned mesh (NEXT-2), the
+                        // other buffers of the z-neighbours' packs (peer memory)
   double chi_floor;
   int* flag;
 };
@@ -290,13 +291,21 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     const int lane = tid & 31;
     int bxyz[3];
     block_coords(g, b, bxyz[0], bxyz[1], bxyz[2]);
+    bxyz[2] += sa.out.bz0[0];                                     // z in the lattice of the whole mesh (NEXT-2)
     const int c0[3] = {cx, cy, cz}, T[3] = {Cfg::TX, Cfg::TY, Cfg::TZ};
+    const int nbl[3] = {g.nb[0], g.nb[1], sa.out.nbz_global};
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       int* L = lists + a * 3 * Cfg::MAXLIST;
       const int l = c0[a] + lane;
       int tb[NG + 1], tl[NG + 1];
-      const int nt = (lane < T[a] && l < g.n) ? push_targets(l, bxyz[a], g.n, g.nb[a], g.bc, tb, tl) : 0;
+      const int nt = (lane < T[a] && l < g.n) ? push_targets(l, bxyz[a], g.n, nbl[a], g.bc, tb, tl) : 0;
+      if (a == 2) {   // z targets: (table entry of the pack that holds the block) << 24 | block z inside that pack
+        for (int q = 0; q < nt; ++q) {
+          const int e = slab_entry(sa.out, tb[q]);
+          tb[q] = (e << 24) | (tb[q] - slab_bz0(sa.out, e));
+        }
+      }
       int incl = nt;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -432,11 +441,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     const int r = (int)(((float)q + 0.5f) * rcx), qx = q - r * ncx;
     const int qz = (int)(((float)r + 0.5f) * rcy), qy = r - qz * ncy;
     const int src = (Lz[qz] * Cfg::TY + Ly[qy]) * Cfg::TX + Lx[qx];
-    const long long tb = ((long long)Lz[Cfg::MAXLIST + qz] * g.nb[1] + Ly[Cfg::MAXLIST + qy]) * g.nb[0] + Lx[Cfg::MAXLIST + qx];
-    double* d = sa.y_out + tb * g.m3 +
+    const int zb = Lz[Cfg::MAXLIST + qz], e = zb >> 24;            // which pack, which block z inside it
+    const long long tb = ((long long)(zb & 0xffffff) * g.nb[1] + Ly[Cfg::MAXLIST + qy]) * g.nb[0] + Lx[Cfg::MAXLIST + qx];
+    double* d = slab_y(sa.out, e) + tb * g.m3 +
                 ((long long)Lz[2 * Cfg::MAXLIST + qz] * g.m + Ly[2 * Cfg::MAXLIST + qy]) * g.m + Lx[2 * Cfg::MAXLIST + qx];
+    const long long efs = slab_fs(sa.out, e);
 #pragma unroll
-    for (int f = 0; f < NF; ++f) d[f * g.fs] = sP[f * Cfg::THREADS + src];
+    for (int f = 0; f < NF; ++f) d[f * efs] = sP[f * Cfg::THREADS + src];
   }
 }
 

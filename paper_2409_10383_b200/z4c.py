@@ -24,6 +24,8 @@ SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_init
            "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
            "z4c_probe_fp64", "z4c_effective_mode", "z4c_time",
            "z4c_restrict", "z4c_prolongate", "z4c_two_level_step",
+           "z4c_set_partition", "z4c_set_neighbor", "z4c_state2", "z4c_stage", "z4c_stage_rhs", "z4c_stage_update",
+           "z4c_constraints_raw",
            "z4c_last_error", "z4c_destroy"]
 
 
@@ -92,6 +94,14 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_restrict.argtypes = [vp, vp, i3]
     L.z4c_prolongate.argtypes = [vp, vp, i3]
     L.z4c_two_level_step.argtypes = [vp, vp, i3, C.c_int]
+    L.z4c_set_partition.argtypes = [vp, C.c_int32, C.c_int32]
+    L.z4c_set_neighbor.argtypes = [vp, C.c_int32, vp, vp, C.c_int32, C.c_int32]
+    L.z4c_state2.argtypes = [vp]
+    L.z4c_state2.restype = C.c_void_p
+    L.z4c_stage.argtypes = [vp, C.c_int]
+    L.z4c_stage_rhs.argtypes = [vp, C.c_int]
+    L.z4c_stage_update.argtypes = [vp, C.c_int]
+    L.z4c_constraints_raw.argtypes = [vp, C.POINTER(C.c_double)]
     L.z4c_time.argtypes = [vp]
     L.z4c_time.restype = C.c_double
     L.z4c_last_error.argtypes = [vp]
@@ -101,7 +111,8 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     for fn in ("z4c_create", "z4c_set_initial_data", "z4c_step", "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior",
                "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync", "z4c_set_variant", "z4c_use_graph",
                "z4c_set_fused", "z4c_step_timed", "z4c_probe_fp64", "z4c_effective_mode", "z4c_restrict", "z4c_prolongate",
-               "z4c_two_level_step"):
+               "z4c_two_level_step", "z4c_set_partition", "z4c_set_neighbor", "z4c_stage", "z4c_stage_rhs", "z4c_stage_update",
+               "z4c_constraints_raw"):
         getattr(L, fn).restype = C.c_int
     if path == default:
         _libs[ng] = L
@@ -306,6 +317,35 @@ class Z4c:
         o = (C.c_int32 * 3)(*[int(v) for v in origin])
         with self.torch.cuda.device(self.device):
             self._check(self.lib.z4c_two_level_step(coarse.h, self.h, o, int(nsteps)))
+
+    # -- NEXT-2: one slab of a partitioned mesh ------------------------------------------------------------
+    def set_partition(self, nbz_global: int, bz0: int):
+        self._check(self.lib.z4c_set_partition(self.h, int(nbz_global), int(bz0)))
+
+    def set_neighbor(self, side: int, d_state: int, d_state2: int, bz0: int, nbz: int):
+        """d_state / d_state2: device addresses (ints) of the neighbour's two state buffers, valid in this process."""
+        self._check(self.lib.z4c_set_neighbor(self.h, int(side), d_state or None, d_state2 or None, int(bz0), int(nbz)))
+
+    def state2_ptr(self) -> int:
+        return int(self.lib.z4c_state2(self.h))
+
+    def stage(self, s: int):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_stage(self.h, int(s)))
+
+    def stage_rhs(self, s: int):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_stage_rhs(self.h, int(s)))
+
+    def stage_update(self, s: int):
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_stage_update(self.h, int(s)))
+
+    def constraints_raw(self) -> np.ndarray:
+        out = (C.c_double * 8)()
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_constraints_raw(self.h, out))
+        return np.array(list(out))
 
     def time(self) -> float:
         return float(self.lib.z4c_time(self.h))
