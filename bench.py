@@ -57,20 +57,31 @@ PAPER_CONTEXT = {"zcps": 1.36e7, "hardware": "NVIDIA A100", "workload": "linear 
                  "gpu_over_cpu_core": ">~200x (PAPER.md:15, 283)"}
 
 
-def workload(name: str):
+def workload_data(name: str, p):
+    """The workload's closed-form initial data on the cells of `p` (any box of the same mesh: a z-slab, NEXT-2)."""
+    if name in ("linear_wave_64", "linear_wave_o6_256"):
+        return I.linear_wave_data(p)
+    if name == "puncture_128":
+        return I.puncture_data(p)
+    if name == "bbh_256":
+        return I.puncture_data(p, (0.5, 0.5), ((3.0, 0.0, 0.0), (-3.0, 0.0, 0.0)))
+    raise SystemExit(f"workload {name} has no per-slab generator")
+
+
+def workload(name: str, params_only: bool = False):
     """(params, initial data on the host, label). Inputs are synthetic and seeded."""
     if name == "linear_wave_64":
         p = I.params_linear_wave(64, 16)
-        return p, I.linear_wave_data(p), WORKLOAD_LABELS[name]
+        return p, None if params_only else I.linear_wave_data(p), WORKLOAD_LABELS[name]
     if name == "puncture_128":
-        p, u, _ = I.config(2)
-        return p, u, WORKLOAD_LABELS[name]
+        p = I.params_puncture(128, 32, 16.0, 2.0)
+        return p, None if params_only else workload_data(name, p), WORKLOAD_LABELS[name]
     if name == "bbh_256":
-        p, u, _ = I.config(3)
-        return p, u, WORKLOAD_LABELS[name]
+        p = I.params_puncture(256, 32, 24.0, 1.0)
+        return p, None if params_only else workload_data(name, p), WORKLOAD_LABELS[name]
     if name == "linear_wave_o6_256":
         p = replace(I.params_linear_wave(256, 64), ng=4)
-        return p, I.linear_wave_data(p), WORKLOAD_LABELS[name]
+        return p, None if params_only else I.linear_wave_data(p), WORKLOAD_LABELS[name]
     if name.startswith("noise_"):            # configs[4] load sweep: noise_<n>_<nbx>x<nby>x<nbz>
         _, n, lat = name.split("_")
         nb = tuple(int(v) for v in lat.split("x"))
@@ -320,16 +331,40 @@ def run_ours(args):
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the Z4c path has no CPU fallback")
+    # fewer GPUs than ranks (a 1-GPU box): the ranks share devices and talk over gloo -- exercises the partitioned
+    # path end to end (CUDA IPC between processes), but the figure is flagged and is no scaling number
+    oversubscribed = world > torch.cuda.device_count()
+    local_rank = local_rank % torch.cuda.device_count()
     torch.cuda.set_device(local_rank)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    build.build()
-    p, u0, label = workload(args.workload)
-    sim = z4c.Z4c(p, device=f"cuda:{local_rank}")
-    sim.set_variant(args.variant)
-    sim.set_fused(args.fuse)
-    sim.use_graph(not args.no_graph)
-    eff_variant, eff_fused = sim.effective_mode()
+        if oversubscribed:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    partitioned = world > 1 and not args.replicas
+    if partitioned:
+        # NEXT-2: ONE mesh, `world` times as long in z, cut into z-slabs -- weak scaling with a real ghost exchange
+        # per stage (peer stores from the stage kernel + one stream-ordered barrier), not independent replicas
+        from paper_2409_10383_b200 import partition as PT
+        p1, _, label = workload(args.workload, params_only=True)
+        pg = replace(p1, nb=(p1.nb[0], p1.nb[1], p1.nb[2] * world))
+        p = PT.slab_params(pg, rank, world)
+        u0 = workload_data(args.workload, p)
+        label = label + f"; mesh extended {world}x along z, one z-slab per rank, ghost images pushed into the neighbour's pack"
+        sim = PT.DistributedSlab(pg, f"cuda:{local_rank}")
+        sim.sim.set_fused(args.fuse)
+        eff_variant, eff_fused = sim.sim.effective_mode()
+    else:
+        p, u0, label = workload(args.workload)
+        sim = z4c.Z4c(p, device=f"cuda:{local_rank}")
+        sim.set_variant(args.variant)
+        sim.set_fused(args.fuse)
+        sim.use_graph(not args.no_graph)
+        eff_variant, eff_fused = sim.effective_mode()
     K, W, R = args.steps, max(args.warmup, 3), max(args.repeats, 1)
     ncells = p.ncells
 
@@ -349,10 +384,13 @@ def run_ours(args):
 
     # ---- per-kernel share of the step (events between kernels, no graph) ------------------------------
     Kt = max(2, min(K, 10))
-    sim.step_timed(2)
-    kt = sim.step_timed(Kt)
+    if partitioned:      # one kernel per stage + the barrier: the step IS the four stage kernels
+        kt = {"rhs": ms_local / K * Kt, "update": 0.0, "ghost": 0.0}
+    else:
+        sim.step_timed(2)
+        kt = sim.step_timed(Kt)
     total_kt = kt["rhs"] + kt["update"] + kt["ghost"]
-    fp64_peak = sim.probe_fp64()
+    fp64_peak = (sim.sim if partitioned else sim).probe_fp64()
     hbm_peak, hbm_src = measured_peaks()
     flops_cell = RHS_FLOPS_PER_CELL if p.ng == 3 else RHS_FLOPS_PER_CELL_O6
     # dominant kernel = the RHS / fused stage kernel, 4 launches per step; its launch time from the graph-replayed
@@ -368,19 +406,21 @@ def run_ours(args):
     h_in = torch.from_numpy(u0).pin_memory()
     h_out = torch.empty_like(h_in).pin_memory()
     Ke = max(3, min(K, 20)) if u0.nbytes < 1e9 else 3
+    core_get = (sim.sim if partitioned else sim).get_interior
     sim.set_initial_data(h_in)
     sim.step(1)
-    sim.get_interior(h_out.numpy())
+    core_get(h_out.numpy())
     barrier()
     t0 = time.perf_counter()
     for _ in range(Ke):
         sim.set_initial_data(h_in)            # H2D of the step's input (synchronises)
         sim.step(1)
-        sim.get_interior(h_out.numpy())       # D2H of the step's result (synchronises)
+        core_get(h_out.numpy())               # D2H of the step's result (synchronises)
     barrier()
     e2e_ms, e2e_units = aggregate((time.perf_counter() - t0) * 1e3, float(ncells) * Ke, dist if world > 1 else None)
     nbytes = int(u0.nbytes)
-    state_mb = (sim.state.numel() + sim.work.numel()) * 8 / 1e6
+    core = sim.sim if partitioned else sim
+    state_mb = (core.state.numel() + core.work.numel()) * 8 / 1e6
     sim.close()
     del sim, h_in, h_out
     torch.cuda.empty_cache()
@@ -405,7 +445,9 @@ def run_ours(args):
             "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": label, "cells_per_gpu": ncells, "blocks": p.nblocks, "n": p.n, "ghosts": g,
-                       "parallelism": "replicas" if world > 1 else "1 GPU",
+                       "parallelism": ("z-slabs of one mesh, peer ghost push + 1 barrier per stage" if partitioned
+                                       else "replicas" if world > 1 else "1 GPU"),
+                       "oversubscribed_ranks_share_gpus": oversubscribed,
                        "l2": "no flush: y+y2+P+Q working set %.0f MB > 126 MB L2" % state_mb,
                        "graph": not args.no_graph, "fuse_mode": eff_fused, "rhs_variant": eff_variant,
                        "requested": {"fuse_mode": args.fuse, "rhs_variant": args.variant}},
@@ -460,6 +502,8 @@ def main():
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--fuse", type=int, default=2, help="0: K2,K3,K1; 1: K2,K3+push; 2: one kernel per RK stage")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--replicas", action="store_true",
+                    help="with --gpus N > 1: N independent packs instead of one mesh partitioned into z-slabs")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # `python bench.py --gpus N` is a complete command: re-launch under torch.distributed.run, one rank per GPU

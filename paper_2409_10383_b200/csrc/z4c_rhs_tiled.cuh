@@ -194,7 +194,11 @@ struct FieldLoop {
     // the first three were waited for up front; the others were probed while the previous field was computed
     if (IT >= 3 && !ready) mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);
     uint32_t ready_next = 1;
+#ifndef Z4C_EXP_NOPROBE
     if (IT + 1 >= 3 && IT + 1 < NF) ready_next = mbar_test_wait(&full[(IT + 1) % Cfg::NSTAGE], ((IT + 1) / Cfg::NSTAGE) & 1);
+#else
+    ready_next = 0;
+#endif
     const double* t = reinterpret_cast<const double*>(tiles + S * Cfg::STAGE_BYTES) + toff;
     if (FULL || active) field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out);
     if (IT + Cfg::NSTAGE < NF) {

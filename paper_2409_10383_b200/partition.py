@@ -157,6 +157,16 @@ class DistributedSlab:
             self.sim.set_neighbor(side, st.data_ptr(), wk.data_ptr() + off2, *self.parts[nb])
         self.barrier()
 
+    @property
+    def stream(self):
+        return self.sim.stream
+
+    def sync(self):
+        self.sim.sync()
+
+    def launch_count(self) -> int:
+        return self.sim.launch_count()
+
     def barrier(self):
         """Every slab has finished what it enqueued so far before any slab runs what comes next."""
         torch, dist = self.torch, self.dist
