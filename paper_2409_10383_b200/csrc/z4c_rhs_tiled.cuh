@@ -40,17 +40,6 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {}
 }
-// Non-blocking probe. Issued one field ahead of its use: the ~100-cycle round trip of the barrier unit then
-// overlaps the stencil work of the current field instead of stalling every warp once per field.
-__device__ __forceinline__ uint32_t mbar_test_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-  return ok;
-}
 __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1,
                                             int c2, int c3, int c4) {
   asm volatile(
@@ -182,25 +171,20 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
   if (Cfg::EARLY_PARK) park_field_early<F>(D, out + (Cfg::E_OFF - Cfg::S_OFF) / 8, Cfg::THREADS);
 }
 
-template <class Cfg, bool FULL, int IT>
+template <class Cfg, int IT>
 struct FieldLoop {
   __device__ __forceinline__ static void run(const CUtensorMap* map, unsigned char* tiles, uint64_t* full,
                                              const int toff, const int cx, const int cy, const int cz, const int b,
-                                             const bool active, const uint32_t ready, double* bw, double* aw,
-                                             const FdConst& fd, const SrcParams& sp, double* u, Derivs& D,
-                                             double* out) {
+                                             const bool active, double* bw, double* aw, const FdConst& fd,
+                                             const SrcParams& sp, double* u, Derivs& D, double* out) {
     constexpr int S = IT % Cfg::NSTAGE;
     constexpr int F = stream_field(IT);
-    // the first three were waited for up front; the others were probed while the previous field was computed
-    if (IT >= 3 && !ready) mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);
-    uint32_t ready_next = 1;
-#ifndef Z4C_EXP_NOPROBE
-    if (IT + 1 >= 3 && IT + 1 < NF) ready_next = mbar_test_wait(&full[(IT + 1) % Cfg::NSTAGE], ((IT + 1) / Cfg::NSTAGE) & 1);
-#else
-    ready_next = 0;
-#endif
+    // Every thread waits on the tile's barrier itself, right before it reads the tile. (Probing the barrier one field
+    // ahead with mbarrier.test_wait and skipping this wait when the probe had already seen the phase complete was
+    // measured: no faster, and on 256^3 runs a few cells per step read stale tile data -- DESIGN.md section 15.)
+    if (IT >= 3) mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);   // the first three were waited for up front
     const double* t = reinterpret_cast<const double*>(tiles + S * Cfg::STAGE_BYTES) + toff;
-    if (FULL || active) field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out);
+    if (active) field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out);
     if (IT + Cfg::NSTAGE < NF) {
       __syncthreads();   // every thread is done reading stage S
       if (threadIdx.x == 0) {
@@ -208,15 +192,14 @@ struct FieldLoop {
         tma_load_5d(tiles + S * Cfg::STAGE_BYTES, map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
       }
     }
-    FieldLoop<Cfg, FULL, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, ready_next, bw, aw, fd, sp, u, D,
-                                      out);
+    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
   }
 };
-template <class Cfg, bool FULL>
-struct FieldLoop<Cfg, FULL, NF> {
+template <class Cfg>
+struct FieldLoop<Cfg, NF> {
   __device__ __forceinline__ static void run(const CUtensorMap*, unsigned char*, uint64_t*, int, int, int, int, int,
-                                             bool, uint32_t, double*, double*, const FdConst&, const SrcParams&,
-                                             double*, Derivs&, double*) {}
+                                             bool, double*, double*, const FdConst&, const SrcParams&, double*,
+                                             Derivs&, double*) {}
 };
 
 // Arguments of the fused stage epilogue (STAGE 1..4): the RK registers, the OTHER state buffer (the stage
@@ -234,8 +217,7 @@ struct StageArgs {
 // STAGE 0: P <- c*P + dt*(F(y) + Q_KO(y)) only (z4c_eval_rhs and the unfused path).
 // STAGE 1..4: K2 + K3 + K1 in one pass ("one kernel per RK stage"): the same recurrence and the same
 // expression forms as k_stage_update, applied to the cell while its 22 values are still in registers.
-// FULL: n is a multiple of every tile edge, so every thread owns a cell (no per-field predication).
-template <class Cfg, int STAGE, bool FULL>
+template <class Cfg, int STAGE>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     k_rhs_tiled(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap pmap,
                 const __grid_constant__ CUtensorMap qmap, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
@@ -258,14 +240,14 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   // padded coordinates of the halo tile's origin = interior coordinates of the tile's first cell
   const int cx = tx * Cfg::TX, cy = ty * Cfg::TY, cz = tz * Cfg::TZ;
   const int i = cx + lx, j = cy + ly, k = cz + lz;
-  const bool active = FULL || (i < g.n && j < g.n && k < g.n);
+  const bool active = i < g.n && j < g.n && k < g.n;
   // gt^{ij} is needed while the very first fields stream in: the six centre values are requested before anything
   // else, so their latency overlaps the barrier set-up and the first tile copies
   double gc[6];
   {
     const double* yc = sa.y_in + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
 #pragma unroll
-    for (int p = 0; p < 6; ++p) gc[p] = active ? __ldg(yc + (GXX + p) * g.fs) : (p == 0 || p == 3 || p == 5 ? 1.0 : 0.0);
+    for (int p = 0; p < 6; ++p) gc[p] = active ? __ldcg(yc + (GXX + p) * g.fs) : (p == 0 || p == 3 || p == 5 ? 1.0 : 0.0);
   }
   if (tid == 0) {
 #pragma unroll
@@ -345,7 +327,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   double* park = reinterpret_cast<double*>(tiles + Cfg::S_OFF) + tid;
   Derivs D;
   derivs_begin(gc, D);
-  FieldLoop<Cfg, FULL, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, 1u, bw, aw, fd, sp, u, D, park);
+  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park);
   double out[NF];
   constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
   if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring
@@ -463,9 +445,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   SM) were slower still (RHS only: 0.183 / 0.219 ms against 0.170 ms): the spills cost more than the warps hide.
 //   8-wide tiles (8x4x4, 8x8x2: 20 % fewer halo bytes) are 20 % slower: 64-byte rows halve the coalescing of the
 //   register / state rows and put two tile rows of a warp on the same shared-memory banks.
-#if defined(Z4C_EXP_TZ)
-using RhsTile = TileCfg<16, 4, Z4C_EXP_TZ, Z4C_EXP_NSTAGE, Z4C_EXP_MINB>;   // tile experiments
-#elif Z4C_NG == 3
+#if Z4C_NG == 3
 using RhsTile = TileCfg<16, 4, 2, 3, 2>;
 #else
 // 4 ghosts: the halo tile grows to 24 x 12 x 10 (23 KB); to keep 2 CTAs per SM the P/Q tiles are read by batched
@@ -523,19 +503,13 @@ struct RegMaps { CUtensorMap p, q; };
 
 // Shared-memory opt-in of every stage instantiation, for the CURRENT device (function attributes are per device:
 // z4c_create calls this once per context, so a process may drive several devices).
-template <class Cfg, int STAGE, bool FULL>
-inline cudaError_t configure_rhs_tiled_one() {
-  constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
-  cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE, FULL>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                              cudaSharedmemCarveoutMaxShared);
-}
 template <class Cfg, int STAGE>
 inline cudaError_t configure_rhs_tiled_stage() {
-  cudaError_t e = configure_rhs_tiled_one<Cfg, STAGE, false>();
-  if (e == cudaSuccess) e = configure_rhs_tiled_one<Cfg, STAGE, true>();
-  return e;
+  constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
+  cudaError_t e = cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_rhs_tiled<Cfg, STAGE>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                              cudaSharedmemCarveoutMaxShared);
 }
 template <class Cfg>
 inline cudaError_t configure_rhs_tiled() {
@@ -555,12 +529,8 @@ inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm,
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
   const long long nblocks = (long long)tx * ty * tz * g.nblk;
   if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  if (g.n % Cfg::TX == 0 && g.n % Cfg::TY == 0 && g.n % Cfg::TZ == 0)
-    k_rhs_tiled<Cfg, STAGE, true><<<(unsigned)nblocks, Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef,
-                                                                                  dt, tx, ty, tz, sa);
-  else
-    k_rhs_tiled<Cfg, STAGE, false><<<(unsigned)nblocks, Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef,
-                                                                                   dt, tx, ty, tz, sa);
+  k_rhs_tiled<Cfg, STAGE><<<(unsigned)nblocks, Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef, dt, tx,
+                                                                          ty, tz, sa);
   return cudaSuccess;
 }
 
