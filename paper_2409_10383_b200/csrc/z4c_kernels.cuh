@@ -286,11 +286,14 @@ __global__ void __launch_bounds__(128) k_stage_update(Pack g, double* __restrict
       const int cx = push_targets(i, bx, g.n, g.nb[0], g.bc, tbx, tlx);
       const int cy = push_targets(j, by, g.n, g.nb[1], g.bc, tby, tly);
       const int cz = push_targets(k, sl.bz0[0] + bz, g.n, sl.nbz_global, g.bc, tbz, tlz);   // global z lattice
+#pragma unroll 1
       for (int a = 0; a < cz; ++a) {
         const int e = slab_entry(sl, tbz[a]);                      // the pack that holds the target block (NEXT-2)
         double* ye = slab_y(sl, e);
         const long long efs = slab_fs(sl, e);
+#pragma unroll 1
         for (int bb = 0; bb < cy; ++bb)
+#pragma unroll 1
           for (int cc = 0; cc < cx; ++cc) {
             if (a + bb + cc == 0) continue;  // the cell itself, already written
             const long long tb = ((long long)(tbz[a] - slab_bz0(sl, e)) * g.nb[1] + tby[bb]) * g.nb[0] + tbx[cc];
