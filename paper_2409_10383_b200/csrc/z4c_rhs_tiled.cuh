@@ -297,22 +297,24 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   // so that no warp arrives late at the first barrier (a serial build by thread 0 cost ~1 us per CTA).
   if (STAGE >= 1 && tid >= Cfg::THREADS - 32) {
     const int lane = tid & 31;
-    int bxyz[3];
-    block_coords(g, b, bxyz[0], bxyz[1], bxyz[2]);
-    bxyz[2] += sa.out.bz0[0];                                     // z in the lattice of the whole mesh (NEXT-2)
-    const int c0[3] = {cx, cy, cz}, T[3] = {Cfg::TX, Cfg::TY, Cfg::TZ};
-    const int nbl[3] = {g.nb[0], g.nb[1], sa.out.nbz_global};
-#pragma unroll
+    int bx, by, bz;
+    block_coords(g, b, bx, by, bz);
+    bz += sa.out.bz0[0];                                          // z in the lattice of the whole mesh (NEXT-2)
+#pragma unroll 1   // one copy of the body for the three axes: off the critical path, and code size is not free here
     for (int a = 0; a < 3; ++a) {
+      const int c0 = a == 0 ? cx : (a == 1 ? cy : cz), T = a == 0 ? Cfg::TX : (a == 1 ? Cfg::TY : Cfg::TZ);
+      const int nbl = a == 0 ? g.nb[0] : (a == 1 ? g.nb[1] : sa.out.nbz_global), bco = a == 0 ? bx : (a == 1 ? by : bz);
       int* L = lists + a * 3 * Cfg::MAXLIST;
-      const int l = c0[a] + lane;
+      const int l = c0 + lane;
       int tb[NG + 1], tl[NG + 1];
-      const int nt = (lane < T[a] && l < g.n) ? push_targets(l, bxyz[a], g.n, nbl[a], g.bc, tb, tl) : 0;
+      const int nt = (lane < T && l < g.n) ? push_targets(l, bco, g.n, nbl, g.bc, tb, tl) : 0;
       if (a == 2) {   // z targets: (table entry of the pack that holds the block) << 24 | block z inside that pack
-        for (int q = 0; q < nt; ++q) {
-          const int e = slab_entry(sa.out, tb[q]);
-          tb[q] = (e << 24) | (tb[q] - slab_bz0(sa.out, e));
-        }
+#pragma unroll
+        for (int q = 0; q < NG + 1; ++q)
+          if (q < nt) {
+            const int e = slab_entry(sa.out, tb[q]);
+            tb[q] = (e << 24) | (tb[q] - slab_bz0(sa.out, e));
+          }
       }
       int incl = nt;
 #pragma unroll
@@ -321,9 +323,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
         if (lane >= o) incl += up;
       }
       const int pos = incl - nt;
-      for (int q = 0; q < nt; ++q) {
-        L[pos + q] = lane; L[Cfg::MAXLIST + pos + q] = tb[q]; L[2 * Cfg::MAXLIST + pos + q] = tl[q];
-      }
+#pragma unroll
+      for (int q = 0; q < NG + 1; ++q)
+        if (q < nt) {
+          L[pos + q] = lane; L[Cfg::MAXLIST + pos + q] = tb[q]; L[2 * Cfg::MAXLIST + pos + q] = tl[q];
+        }
       if (lane == 31) lists[9 * Cfg::MAXLIST + a] = incl;
     }
   }
@@ -331,10 +335,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   if (STAGE >= 2 && !Cfg::PQ_TMA && active && lx == 0) {
     // ask L2 for this tile's rows of the RK registers (one 128-byte line per row and field)
     const long long c0 = (long long)b * g.n3 + ((long long)k * g.n + j) * g.n + i;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      asm volatile("prefetch.global.L2 [%0];" ::"l"(sa.Q + c0 + f * g.is));
-      if (STAGE >= 3) asm volatile("prefetch.global.L2 [%0];" ::"l"(Preg + c0 + f * g.is));
+    const double* pq = sa.Q + c0;
+    const double* pp = Preg + c0;
+#pragma unroll 1   // a real loop: this kernel is instruction-fetch bound, straight-line code is not free
+    for (int f = 0; f < NF; ++f, pq += g.is, pp += g.is) {
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(pq));
+      if (STAGE >= 3) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp));
     }
   }
   double bw[3], aw[3];
