@@ -185,6 +185,12 @@ static int enforce_global(const Params& P, double* u, int do_enforce) {
 // ---- O6 RK4, 3-register recurrence -------------------------------------------------------
 // One stage of the recurrence on n values: L = F(y) + Q_KO(y) of the current y. (One function so that the
 // single-level and the two-level drivers run the very same statements.)
+// Reading O6 (amended in round 2): the two factors 1/6 of the recurrence are applied as a multiplication by the
+// correctly rounded double 1/6, not as a division. The paper prints no recurrence at all ("a family of
+// explicit Runge-Kutta methods"; RK4 at PAPER.md:169, 203, 279), so which of the two equal real-number forms is used is
+// ours to fix; the product costs the GPU one instruction where the IEEE division costs ~15 in each of 44 places, in
+// kernels that are instruction-fetch bound. Oracle and kernels use the same form, each rounding product and sum separately.
+static const double SIXTH = 1.0 / 6.0;
 static void rk_stage_update(int stage, size_t n, double dt, const double* L, double* y, double* Pr, double* Q) {
   if (stage == 1) {
     // stage 1: P = L(y); Q = P; y = E(y + P/2)
@@ -195,12 +201,12 @@ static void rk_stage_update(int stage, size_t n, double dt, const double* L, dou
       y[q] = y[q] + 0.5 * Pr[q];
     }
   } else if (stage == 2) {
-    // stage 2: P = L(y); y = E(y + (P-Q)/2); Q = Q/6
+    // stage 2: P = L(y); y = E(y + (P-Q)/2); Q = Q * (1/6)
 #pragma omp parallel for schedule(static)
     for (long long q = 0; q < (long long)n; ++q) {
       Pr[q] = dt * L[q];
       y[q] = y[q] + 0.5 * (Pr[q] - Q[q]);
-      Q[q] = Q[q] / 6.0;
+      Q[q] = Q[q] * SIXTH;
     }
   } else if (stage == 3) {
     // stage 3: P = L(y) - P/2; y = E(y + P); Q = Q - P
@@ -211,11 +217,11 @@ static void rk_stage_update(int stage, size_t n, double dt, const double* L, dou
       Q[q] = Q[q] - Pr[q];
     }
   } else {
-    // stage 4: P = L(y) + 2P; y = E(y + (Q + P/6))
+    // stage 4: P = L(y) + 2P; y = E(y + (Q + P * (1/6)))
 #pragma omp parallel for schedule(static)
     for (long long q = 0; q < (long long)n; ++q) {
       Pr[q] = dt * L[q] + 2.0 * Pr[q];
-      y[q] = y[q] + (Q[q] + Pr[q] / 6.0);
+      y[q] = y[q] + (Q[q] + Pr[q] * SIXTH);
     }
   }
 }

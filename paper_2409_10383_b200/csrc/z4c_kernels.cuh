@@ -207,11 +207,15 @@ __device__ __forceinline__ bool any_nonfinite(const double* u) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// The two factors 1/6 of the recurrence: a product with the correctly rounded double 1/6 (reading O6 as amended in
+// round 2), product and sum rounded separately, as in the oracle.
+__device__ constexpr double SIXTH = 1.0 / 6.0;
+
 // K3: RK4 stage update in the 3-register recurrence (O6) + enforcement (O7), interior cells.
 //   stage 1: Q = P;  y = E(y + P/2)
-//   stage 2: y = E(y + (P - Q)/2);  Q = Q/6
+//   stage 2: y = E(y + (P - Q)/2);  Q = Q * (1/6)
 //   stage 3: y = E(y + P);  Q = Q - P
-//   stage 4: y = E(y + (Q + P/6))
+//   stage 4: y = E(y + (Q + P * (1/6)))
 //   stage 0: y = E(y)                               (z4c_enforce / z4c_set_initial_data)
 // One thread per cell; every access is a run of n consecutive doubles per (j,k) row.
 // ---------------------------------------------------------------------------------------------
@@ -261,14 +265,14 @@ __global__ void __launch_bounds__(128) k_stage_update(Pack g, double* __restrict
       } else if (STAGE == 2) {
         const double Q = qc[f * g.is];
         u[f] = u[f] + 0.5 * (P - Q);
-        qc[f * g.is] = Q / 6.0;
+        qc[f * g.is] = __dmul_rn(Q, SIXTH);
       } else if (STAGE == 3) {
         const double Q = qc[f * g.is];
         u[f] = u[f] + P;
         qc[f * g.is] = Q - P;
       } else {
         const double Q = qc[f * g.is];
-        u[f] = u[f] + (Q + P / 6.0);
+        u[f] = u[f] + __dadd_rn(Q, __dmul_rn(P, SIXTH));
       }
     }
   }

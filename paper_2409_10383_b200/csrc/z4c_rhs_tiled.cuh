@@ -421,7 +421,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
         const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
         pc[f * g.is] = P;
         u[f] = u[f] + 0.5 * (P - Q);
-        qc[f * g.is] = Q / 6.0;
+        qc[f * g.is] = __dmul_rn(Q, SIXTH);
       } else if (STAGE == 3) {
         const double P = -0.5 * (Cfg::PQ_TMA ? sP[f * Cfg::THREADS + tid] : Pold[f]) + dt * out[f];
         const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
@@ -431,7 +431,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
       } else {
         const double P = 2.0 * (Cfg::PQ_TMA ? sP[f * Cfg::THREADS + tid] : Pold[f]) + dt * out[f];
         const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
-        u[f] = u[f] + (Q + P / 6.0);
+        u[f] = u[f] + __dadd_rn(Q, __dmul_rn(P, SIXTH));
       }
     }
     bool bad = enforce_cell(u, sa.chi_floor);
