@@ -226,8 +226,8 @@ __device__ __forceinline__ int push_targets(int l, int bcoord, int n, int nbl, i
   int c = 0;
   tb[c] = bcoord; tl[c] = l + NG; ++c;
   if (bc == 0) {
-    if (l < NG) { tb[c] = (bcoord + nbl - 1) % nbl; tl[c] = l + n + NG; ++c; }
-    else if (l >= n - NG) { tb[c] = (bcoord + 1) % nbl; tl[c] = l - n + NG; ++c; }
+    if (l < NG) { tb[c] = bcoord == 0 ? nbl - 1 : bcoord - 1; tl[c] = l + n + NG; ++c; }
+    else if (l >= n - NG) { tb[c] = bcoord + 1 == nbl ? 0 : bcoord + 1; tl[c] = l - n + NG; ++c; }
   } else {
     if (l < NG) {
       if (bcoord > 0) { tb[c] = bcoord - 1; tl[c] = l + n + NG; ++c; }

@@ -243,7 +243,7 @@ template <class Cfg, int STAGE>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     k_rhs_tiled(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap pmap,
                 const __grid_constant__ CUtensorMap qmap, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
-                double c, double dt, int tiles_x, int tiles_y, int tiles_z, StageArgs sa) {
+                double c, double dt, int tiles_y, int b0, StageArgs sa) {
   static_assert(Cfg::NSTAGE >= 3, "the three shift components are staged together");
   extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
   uint64_t* full = reinterpret_cast<uint64_t*>(tiles + Cfg::BAR_OFF);
@@ -254,11 +254,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   int* lists = reinterpret_cast<int*>(tiles + Cfg::LIST_OFF);
   const int tid = threadIdx.x;
   const int lx = tid % Cfg::TX, ly = (tid / Cfg::TX) % Cfg::TY, lz = tid / (Cfg::TX * Cfg::TY);
-  int t = blockIdx.x;
-  const int tx = t % tiles_x; t /= tiles_x;
-  const int ty = t % tiles_y; t /= tiles_y;
-  const int tz = t % tiles_z; t /= tiles_z;
-  const int b = t;
+  // grid = (tiles_x, tiles_y * tiles_z, blocks of this launch): one integer division per CTA instead of three
+  const int tx = blockIdx.x, tz = blockIdx.y / tiles_y, ty = blockIdx.y - tz * tiles_y;
+  const int b = b0 + blockIdx.z;
   // padded coordinates of the halo tile's origin = interior coordinates of the tile's first cell
   const int cx = tx * Cfg::TX, cy = ty * Cfg::TY, cz = tz * Cfg::TZ;
   const int i = cx + lx, j = cy + ly, k = cz + lz;
@@ -555,10 +553,12 @@ inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm,
                                       const StageArgs& sa) {
   constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
-  const long long nblocks = (long long)tx * ty * tz * g.nblk;
-  if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  k_rhs_tiled<Cfg, STAGE><<<(unsigned)nblocks, Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef, dt, tx,
-                                                                          ty, tz, sa);
+  if ((long long)ty * tz > 65535) return cudaErrorInvalidConfiguration;
+  for (int b0 = 0; b0 < g.nblk; b0 += 65535) {   // gridDim.z <= 65535: packs with more blocks take several launches
+    const int nb = g.nblk - b0 < 65535 ? g.nblk - b0 : 65535;
+    k_rhs_tiled<Cfg, STAGE><<<dim3(tx, ty * tz, nb), Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef, dt, ty,
+                                                                                b0, sa);
+  }
   return cudaSuccess;
 }
 
