@@ -86,3 +86,23 @@ def test_reference_arm_prints_contract_line():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["unit"] == "zone-cycles/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_workload_params_and_slab_data_agree_with_the_configs():
+    """bench.py's per-slab generators (NEXT-2 weak scaling) give the same cells as the whole-mesh generators."""
+    from dataclasses import replace
+    import numpy as np
+    import bench
+    from paper_2409_10383_b200 import inputs as I
+    from paper_2409_10383_b200 import partition as PT
+    for idx, name in ((2, "puncture_128"), (3, "bbh_256")):
+        p_cfg = I.config(idx)[0] if idx == 2 else None
+        p, _, _ = bench.workload(name, params_only=True)
+        if p_cfg is not None:
+            assert p == p_cfg
+    # a shrunk two-puncture mesh: whole-mesh data cut into z-slabs == data generated slab by slab
+    p = replace(bench.workload("bbh_256", params_only=True)[0], n=8, nb=(2, 2, 4), dx=0.75, xmin=(-6.0, -6.0, -12.0))
+    whole = bench.workload_data("bbh_256", p)
+    for r in range(3):
+        ps = PT.slab_params(p, r, 3)
+        assert np.array_equal(bench.workload_data("bbh_256", ps), PT.slab_interior(whole, p, r, 3))
