@@ -357,13 +357,12 @@ __global__ void __launch_bounds__(K4_THREADS)
     const double* yc = y + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
     double u[NF], out[NF], c[6];
     Derivs D;
-    gather_global<true>(yc, g.fs, g.m, g.m2, fd, sp, u, D, out);
-    double dA[3][6];
+    gather_global<false>(yc, g.fs, g.m, g.m2, fd, sp, u, D, out);
+    const int st[3] = {1, g.m, g.m2};
+    z4c_constraints_point(u, D, [&](const int a, double* q) {
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-      for (int p = 0; p < 6; ++p) dA[a][p] = D.d1[AXX + p][a];
-    z4c_constraints_point(u, D, dA, c);
+      for (int p = 0; p < 6; ++p) q[p] = d1_raw(yc + (AXX + p) * g.fs, st[a]) * fd.inv12h;
+    }, c);
     if (percell) {
       int bx, by, bz;
       block_coords(g, b, bx, by, bz);

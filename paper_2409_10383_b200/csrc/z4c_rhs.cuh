@@ -248,9 +248,11 @@ __device__ __forceinline__ void z4c_sources_post(const SrcParams& P, const doubl
   for (int i = 0; i < 3; ++i) out[BETAX + i] += P.shift_gamma * u[GAMX + i] - P.shift_eta * u[BETAX + i];
 }
 
-// O5 constraints: c = {H, M_x, M_y, M_z, |M|^2, |Z|^2}. dA[k][p] = centred d_k At_p.
-__device__ __forceinline__ void z4c_constraints_point(const double* u, const Derivs& D, const double (&dA)[3][6],
-                                                      double* c) {
+// O5 constraints: c = {H, M_x, M_y, M_z, |M|^2, |Z|^2}. dAt(i, q) returns the centred d_i At_p, p = 0..5, of axis i in
+// q[6]: the 18 derivatives of At_ij are asked for one axis at a time (6 live values instead of 18, which together with
+// the geometry did not fit the register file: 552 bytes of spill in round 1).
+template <class DA>
+__device__ __forceinline__ void z4c_constraints_point(const double* u, const Derivs& D, DA dAt, double* c) {
   Geom G;
   geometry(u, D, G);
   const double* g = u + GXX;
@@ -260,10 +262,14 @@ __device__ __forceinline__ void z4c_constraints_point(const double* u, const Der
   c[0] = G.Rscal - G.AA + (2.0 / 3.0) * G.K * G.K;
   double M[3];
 #pragma unroll
-  for (int j = 0; j < 3; ++j) {
-    double s = 0.0;
+  for (int j = 0; j < 3; ++j) M[j] = -(2.0 / 3.0) * (D.d1[KHAT][j] + 2.0 * D.d1[THETA][j]);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
+  for (int i = 0; i < 3; ++i) {
+    double dAi[6];
+    dAt(i, dAi);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double s = 0.0;
       // d_i At^i_j = (d_i gt^{ik}) At_kj + gt^{ik} d_i At_kj,  d_i gt^{ik} = - gt^{ic} d_i gt_cd gt^{dk}
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
@@ -272,15 +278,15 @@ __device__ __forceinline__ void z4c_constraints_point(const double* u, const Der
         for (int cc = 0; cc < 3; ++cc)
 #pragma unroll
           for (int d = 0; d < 3; ++d) dginv -= gi[sym(i, cc)] * D.d1[GXX + sym(cc, d)][i] * gi[sym(d, k)];
-        s += dginv * A[sym(k, j)] + gi[sym(i, k)] * dA[i][sym(k, j)];
+        s += dginv * A[sym(k, j)] + gi[sym(i, k)] * dAi[sym(k, j)];
         s += G.Gu[i][sym(i, k)] * G.Am[k][j] - G.Gu[k][sym(i, j)] * G.Am[i][k];
       }
       s -= 1.5 * G.Am[i][j] * D.d1[CHI][i] * ichi;
+      M[j] += s;
     }
-    s -= (2.0 / 3.0) * (D.d1[KHAT][j] + 2.0 * D.d1[THETA][j]);
-    M[j] = s;
-    c[1 + j] = s;
   }
+#pragma unroll
+  for (int j = 0; j < 3; ++j) c[1 + j] = M[j];
   double Z[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) Z[i] = u[GAMX + i] - G.Gd[i];
