@@ -200,12 +200,18 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
   if (Cfg::EARLY_PARK) park_field_early<F>(D, out + (Cfg::E_OFF - Cfg::S_OFF) / 8, Cfg::THREADS);
 }
 
+// the field after which the RK-register tiles are asked for (they are needed only in the epilogue; asked for at kernel
+// start they queue ahead of the first ring refills)
+#ifndef Z4C_PQ_AT
+#define Z4C_PQ_AT 6
+#endif
 template <class Cfg, int IT>
 struct FieldLoop {
+  template <class LATE>
   __device__ __forceinline__ static void run(const CUtensorMap* map, unsigned char* tiles, uint64_t* full,
                                              const int toff, const int cx, const int cy, const int cz, const int b,
                                              const bool active, double* bw, double* aw, const FdConst& fd,
-                                             const SrcParams& sp, double* u, Derivs& D, double* out) {
+                                             const SrcParams& sp, double* u, Derivs& D, double* out, LATE late) {
     constexpr int S = IT % Cfg::NSTAGE;
     constexpr int F = stream_field(IT);
     // Every thread waits on the tile's barrier itself, right before it reads the tile. (Probing the barrier one field
@@ -220,17 +226,19 @@ struct FieldLoop {
         if (elect_one()) {
           mbar_expect_tx(&full[S], Cfg::TILE_BYTES);
           tma_load_5d(tiles + S * Cfg::STAGE_BYTES, map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
+          if (IT == Z4C_PQ_AT) late();
         }
       }
     }
-    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out);
+    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out, late);
   }
 };
 template <class Cfg>
 struct FieldLoop<Cfg, NF> {
+  template <class LATE>
   __device__ __forceinline__ static void run(const CUtensorMap*, unsigned char*, uint64_t*, int, int, int, int, int,
                                              bool, double*, double*, const FdConst&, const SrcParams&, double*,
-                                             Derivs&, double*) {}
+                                             Derivs&, double*, LATE) {}
 };
 
 // Arguments of the fused stage epilogue (STAGE 1..4): the RK registers, the OTHER state buffer (the stage
@@ -291,12 +299,6 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     for (int s = 0; s < Cfg::NSTAGE; ++s) {
       mbar_expect_tx(&full[s], Cfg::TILE_BYTES);
       tma_load_5d(tiles + s * Cfg::STAGE_BYTES, &map, &full[s], cx, cy, cz, b, stream_field(s));
-    }
-    // the RK registers of this tile, all 22 fields in one box each: they land long before the epilogue needs them
-    if (STAGE >= 2 && Cfg::PQ_TMA) {
-      mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
-      tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
-      if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
     }
   }
   // push lists (O2): per axis, every (source cell of this tile -> destination block, padded index) pair, the
@@ -363,7 +365,14 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   double* park = reinterpret_cast<double*>(tiles + Cfg::S_OFF) + tid;
   Derivs D;
   derivs_begin(gc, D);
-  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park);
+  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park, [&]() {
+    // the RK registers of this tile, all 22 fields in one box each (run by the one elected thread)
+    if (STAGE >= 2 && Cfg::PQ_TMA) {
+      mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
+      tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
+      if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
+    }
+  });
   double out[NF];
   constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
   if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring

@@ -148,3 +148,21 @@ def test_two_level_argument_checks(Z):
         bad_dt.two_level_step(coarse, (0, 0, 0), 1)
     for s in (coarse, fine, other, bad_dx, bad_dt):
         s.close()
+
+
+def test_two_level_step_with_four_ghosts(Z, oracle):
+    """The paper's production scheme on the refined-corner wave: 4 ghosts, 6th-order stencils, 5-node interpolation
+    ("5th order for 4 ghost"), 2 steps, both levels at 1e-12."""
+    pc = replace(I.params_linear_wave(32, 16), cfl=0.125, ng=4)
+    pf = replace(pc, nb=(2, 2, 2), dx=pc.dx / 2, cfl=0.25, bc=1)
+    uc, uf = I.linear_wave_data(pc), I.linear_wave_data(pf)
+    coarse, fine = levels(Z, pc, pf, uc, uf)
+    rc, rf, bad = oracle.step_two_level(pc, pf, 16, (0, 0, 0), oracle.enforce(pc, uc)[0], oracle.enforce(pf, uf)[0], 2)
+    assert bad == 0
+    fine.two_level_step(coarse, (0, 0, 0), 2)
+    for sim, ref, p in ((coarse, rc, pc), (fine, rf, pf)):
+        sim.sync()
+        err = rel_err(sim.get_interior(), ref, perturbation_scale(ref, p))
+        assert err.max() <= 1e-12, dict(zip(I.FIELD_NAMES, err))
+    coarse.close()
+    fine.close()
