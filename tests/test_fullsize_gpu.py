@@ -230,6 +230,36 @@ def test_64bit_indexing_pack_larger_than_2_31_elements(Z):
     torch.cuda.empty_cache()
 
 
+def test_pack_with_more_blocks_than_one_grid_dimension_holds(Z):
+    """The stage kernel runs on a 3-D grid with the block index in gridDim.z (<= 65535): a pack of 72,000 blocks of 6^3
+    takes two launches per stage. Periodic-tiling invariance against the 8-block pack, compared on the device."""
+    import torch
+    tile = (2, 2, 2)
+    p = I.params_noise(6, (50, 40, 36), 0.1)
+    assert p.nblocks == 72000
+    ps = replace(p, nb=tile)
+    base = torch.from_numpy(I.noise_data(ps, 77)).cuda()
+    small = Z.Z4c(ps)
+    small.set_initial_data(base)
+    small.step(2)
+    small.sync()
+    ref = torch.empty_like(base)
+    small.get_interior(ref)
+    small.close()
+    u = base.repeat(1, p.nb[2] // 2, p.nb[1] // 2, p.nb[0] // 2).contiguous()
+    big = Z.Z4c(p)
+    assert big.effective_mode() == (0, 2)
+    big.set_initial_data(u)
+    big.step(2)
+    big.sync()
+    big.get_interior(u)
+    v = u.view(I.NF, p.nb[2] // 2, 12, p.nb[1] // 2, 12, p.nb[0] // 2, 12)
+    assert bool(torch.equal(v, ref.view(I.NF, 1, 12, 1, 12, 1, 12).expand_as(v)))
+    big.close()
+    del u, base, ref, v
+    torch.cuda.empty_cache()
+
+
 def test_zero_steps_and_reinitialisation(Z):
     p = I.params_noise(16, (1, 1, 2))
     u = I.noise_data(p, 7)
