@@ -79,19 +79,28 @@ struct TileCfg {
   // field is done, so they stay out of registers through the whole field stream)
   static constexpr bool EARLY_PARK = EARLY_PARK_;
   static constexpr int E_OFF = S_OFF + REG_BYTES;
-  static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0);   // push lists
+  // two-pass mixed derivatives: planes of D_x u and D_y u of the current field (raw, unscaled) on the tile plus the rows
+  // / planes the second pass reaches, R = NG - 1 cells on either side. With PQ_TMA they live in the P/Q tile area, which
+  // is idle until the field stream ends (the RK-register tiles are asked for after the last field); else in their own area.
+  static constexpr int MIX_R = NG - 1;
+  static constexpr int PXY = TY + 2 * MIX_R, PZ = TZ + 2 * MIX_R;
+  static constexpr int PX_PLANE = PXY * TX, PX_ELEMS = PZ * PX_PLANE, PY_PLANE = TY * TX, PY_ELEMS = PZ * PY_PLANE;
+  static constexpr int MIX_BYTES = ((PX_ELEMS + PY_ELEMS) * 8 + 127) / 128 * 128;
+  static constexpr int SCR_OFF = PQ_TMA ? P_OFF : E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0);
+  static_assert(!PQ_TMA || MIX_BYTES <= 2 * REG_BYTES, "the planes fit the P/Q tile area");
+  static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0) + (PQ_TMA ? 0 : MIX_BYTES);   // push lists
   static constexpr int MAXLIST = 32;
   static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
   static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
   static_assert(TX + 2 * NG <= MAXLIST && TY + 2 * NG <= MAXLIST && TZ + 2 * NG <= MAXLIST, "push list size");
 };
 
-// Field streaming order: the shift first (its sign and size weight every other field's advection); then the
-// fields with second derivatives (67 shared-memory loads each) alternate with the advection-only fields (19 loads),
-// so that the ring drains at an even rate and no tile is asked for before its copy has landed.
+// Field streaming order: fields with second derivatives (two passes over the tile, a barrier in between) alternate with
+// the others (one pass), so that the ring drains at an even rate and the single set of D_x / D_y planes is never
+// rewritten before every thread has finished reading it (a whole field, with its barrier, lies in between).
 __host__ __device__ constexpr int stream_field(int it) {
-  constexpr int order[NF] = {BETAX, BETAY, BETAZ, CHI,  GXX,  AXX,  GXY,  AXY,  GXZ,  AXZ,   GYY,
-                             AYY,   GYZ,   AYZ,   GZZ,  AZZ,  ALPHA, KHAT, GAMX, GAMY, GAMZ, THETA};
+  constexpr int order[NF] = {BETAX, AXX,  BETAY, AXY,  BETAZ, AXZ,  CHI,  AYY,  GXX,  AYZ,  GXY,
+                             AZZ,   GXZ,  KHAT,  GYY,  GAMX,  GYZ,  GAMY, GZZ,  GAMZ, ALPHA, THETA};
   return order[it];
 }
 
@@ -105,7 +114,7 @@ __host__ __device__ constexpr bool wants_dform(int f) { return f <= GZZ || f == 
 // One axis of one field out of the shared-memory tile. t points at the cell, S is the compile-time stride.
 template <int S, bool WANT_D1, bool WANT_D2, bool DFORM>
 __device__ __forceinline__ void axis_tile(const double* t, const double c, const double bw, const double aw,
-                                          const FdConst& fd, double& d1, double& d2, double& adv) {
+                                          const FdConst& fd, double& d1, double& d2, double& adv, double& raw1) {
 #if Z4C_NG == 3
   const double lm3 = t[-3 * S], lm2 = t[-2 * S], lm1 = t[-S], lp1 = t[S], lp2 = t[2 * S], lp3 = t[3 * S];
   const double e1 = lp1 - lm1, e2 = lp2 - lm2, e3 = lp3 - lm3;
@@ -119,7 +128,8 @@ __device__ __forceinline__ void axis_tile(const double* t, const double c, const
     if (WANT_D2) d2 = (16.0 * t1 - t2 - 30.0 * c) * fd.inv12h2;
     k = t3 - 6.0 * t2 + 15.0 * t1 - 20.0 * c;
   }
-  if (WANT_D1) d1 = (8.0 * e1 - e2) * fd.inv12h;
+  raw1 = 8.0 * e1 - e2;   // the centred first derivative before scaling: also the first pass of the mixed derivatives
+  if (WANT_D1) d1 = raw1 * fd.inv12h;
   const double sy = e3 - 6.0 * e2 + 21.0 * e1;
 #else
   // 6th order (NEXT-1). The lopsided pair obeys the same identity as at 4th order:
@@ -138,32 +148,35 @@ __device__ __forceinline__ void axis_tile(const double* t, const double c, const
     if (WANT_D2) d2 = (270.0 * t1 - 27.0 * t2 + 2.0 * t3 - 490.0 * c) * fd.inv12h2;
     k = 56.0 * t1 - 28.0 * t2 + 8.0 * t3 - t4 - 70.0 * c;
   }
-  if (WANT_D1) d1 = (45.0 * e1 - 9.0 * e2 + e3) * fd.inv12h;
+  raw1 = 45.0 * e1 - 9.0 * e2 + e3;
+  if (WANT_D1) d1 = raw1 * fd.inv12h;
   const double sy = 104.0 * e1 - 32.0 * e2 + 8.0 * e3 - e4;
 #endif
   // bw = c_adv beta/(24h) [120h], aw = c_adv |beta|/(24h) + eps/(64h) [.., 256h]: advection and dissipation in two FMAs
   adv += bw * sy + aw * k;
 }
 
-// mixed second derivative from the tile, compile-time strides
-template <int SA, int SB>
-__device__ __forceinline__ double mixed_tile(const double* t) {
+// centred first derivative, raw (unscaled), along a compile-time stride: the operator that is applied twice
+template <int S>
+__device__ __forceinline__ double d1_tile(const double* q) {
 #if Z4C_NG == 3
-  auto inner = [&](const double* q) { return 8.0 * (q[SA] - q[-SA]) - (q[2 * SA] - q[-2 * SA]); };
-  return 8.0 * (inner(t + SB) - inner(t - SB)) - (inner(t + 2 * SB) - inner(t - 2 * SB));
+  return 8.0 * (q[S] - q[-S]) - (q[2 * S] - q[-2 * S]);
 #else
-  auto inner = [&](const double* q) {
-    return 45.0 * (q[SA] - q[-SA]) - 9.0 * (q[2 * SA] - q[-2 * SA]) + (q[3 * SA] - q[-3 * SA]);
-  };
-  return 45.0 * (inner(t + SB) - inner(t - SB)) - 9.0 * (inner(t + 2 * SB) - inner(t - 2 * SB)) +
-         (inner(t + 3 * SB) - inner(t - 3 * SB));
+  return 45.0 * (q[S] - q[-S]) - 9.0 * (q[2 * S] - q[-2 * S]) + (q[3 * S] - q[-3 * S]);
 #endif
 }
 
-template <class Cfg, int F>
+// One field out of its shared-memory tile. Fields with second derivatives take TWO passes: pass 1 (every thread, also
+// the ones whose cell lies outside the block: their rows are somebody's neighbours) takes the axis stencils and stores
+// D_x u and D_y u of its own cell and of the 2R rows / planes around the tile into the plane set `scr`; `release()` is
+// the CTA barrier (after which nobody reads the tile any more, so it also frees the ring slot); pass 2 takes D_y and
+// D_z of those planes: D_xy = D_y(D_x u), D_xz = D_z(D_x u), D_yz = D_z(D_y u) -- the same operator applied twice, in the
+// same order and form as the one-pass evaluation (bit-identical), at 32 + 7 instead of 48 shared-memory accesses and
+// 24 instead of 48 FP64 instructions per field (63 + 10 instead of 108, 53 instead of 141 at 6th order).
+template <class Cfg, int F, class REL>
 __device__ __forceinline__ void field_from_tile(const double* t, const double* bw, const double* aw,
                                                 const FdConst& fd, const SrcParams& sp, double* u, Derivs& D,
-                                                double* out) {
+                                                double* out, double* scr, const int ly, const int lz, REL release) {
   constexpr bool W1 = need_d1(F), W2 = need_d2(F);
   const double c = t[0];
   u[F] = c;
@@ -183,62 +196,114 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
     }
   }
   constexpr bool DF = wants_dform(F);
-  axis_tile<1, W1, W2, DF>(t, c, w1[0], w2[0], fd, d1x, d2x, adv);
-  axis_tile<Cfg::SY, W1, W2, DF>(t, c, w1[1], w2[1], fd, d1y, d2y, adv);
-  axis_tile<Cfg::SZ, W1, W2, DF>(t, c, w1[2], w2[2], fd, d1z, d2z, adv);
+  double rx, ry, rz;
+  axis_tile<1, W1, W2, DF>(t, c, w1[0], w2[0], fd, d1x, d2x, adv, rx);
+  axis_tile<Cfg::SY, W1, W2, DF>(t, c, w1[1], w2[1], fd, d1y, d2y, adv, ry);
+  axis_tile<Cfg::SZ, W1, W2, DF>(t, c, w1[2], w2[2], fd, d1z, d2z, adv, rz);
   if (W1) { D.d1[F][0] = d1x; D.d1[F][1] = d1y; D.d1[F][2] = d1z; }
   if (W2) {
+    static_assert(Cfg::TY == 4 && Cfg::TZ == 2, "the halo-row assignment below is written for 16 x 4 x 2 tiles");
+    constexpr int R = Cfg::MIX_R;
+    double* px = scr + ((lz + R) * Cfg::PXY + (ly + R)) * Cfg::TX + (threadIdx.x % Cfg::TX);
+    double* py = scr + Cfg::PX_ELEMS + ((lz + R) * Cfg::TY + ly) * Cfg::TX + (threadIdx.x % Cfg::TX);
+    // every tile load first, every store after: the compiler cannot know that tile, planes and parking area are disjoint
+#if Z4C_NG == 3
+    const int dy = ly < R ? -R : R;   // rows -2, -1 (threads ly = 0, 1) and 4, 5 (ly = 2, 3) of the tile's own planes
+    const double hxy = d1_tile<1>(t + dy * Cfg::SY);
+    double hxz[2], hyz[2];            // planes -2, -1 (lz = 0, 1 with dz = -2) and 2, 3 (dz = +2)
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      hxz[q] = d1_tile<1>(t + (2 * q - 1) * R * Cfg::SZ);
+      hyz[q] = d1_tile<Cfg::SY>(t + (2 * q - 1) * R * Cfg::SZ);
+    }
+    out[F * Cfg::THREADS] = adv;
+    px[0] = rx;
+    py[0] = ry;
+    px[dy * Cfg::TX] = hxy;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      px[(2 * q - 1) * R * Cfg::PX_PLANE] = hxz[q];
+      py[(2 * q - 1) * R * Cfg::PY_PLANE] = hyz[q];
+    }
+#else
+    double hxy[2], hxz[3], hyz[3];
+#pragma unroll
+    for (int q = 0; q < 2; ++q)       // rows -3..0 and 3..6 (rows 0 and 3 are rewritten with the same value)
+      hxy[q] = d1_tile<1>(t + (2 * q - 1) * R * Cfg::SY);
+    const int dzm = lz == 0 ? -1 : 1;  // planes -3, -2 | 3, 4 | -1 (lz = 0), 2 (lz = 1)
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const int dz = q == 0 ? -R : (q == 1 ? R : dzm);
+      hxz[q] = d1_tile<1>(t + dz * Cfg::SZ);
+      hyz[q] = d1_tile<Cfg::SY>(t + dz * Cfg::SZ);
+    }
+    out[F * Cfg::THREADS] = adv;
+    px[0] = rx;
+    py[0] = ry;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) px[(2 * q - 1) * R * Cfg::TX] = hxy[q];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const int dz = q == 0 ? -R : (q == 1 ? R : dzm);
+      px[dz * Cfg::PX_PLANE] = hxz[q];
+      py[dz * Cfg::PY_PLANE] = hyz[q];
+    }
+#endif
+    release();
     double d2[6];
     d2[sym(0, 0)] = d2x; d2[sym(1, 1)] = d2y; d2[sym(2, 2)] = d2z;
-    d2[sym(0, 1)] = mixed_tile<1, Cfg::SY>(t) * fd.inv144h2;
-    d2[sym(0, 2)] = mixed_tile<1, Cfg::SZ>(t) * fd.inv144h2;
-    d2[sym(1, 2)] = mixed_tile<Cfg::SY, Cfg::SZ>(t) * fd.inv144h2;
+    d2[sym(0, 1)] = d1_tile<Cfg::TX>(px) * fd.inv144h2;
+    d2[sym(0, 2)] = d1_tile<Cfg::PX_PLANE>(px) * fd.inv144h2;
+    d2[sym(1, 2)] = d1_tile<Cfg::PY_PLANE>(py) * fd.inv144h2;
     consume_d2<F>(d2, D);
+  } else {
+    // parked in shared memory until the sources are assembled: 22 doubles fewer live through the tensor algebra
+    out[F * Cfg::THREADS] = adv;
   }
-  // parked in shared memory until the sources are assembled: 22 doubles fewer live through the tensor algebra
-  out[F * Cfg::THREADS] = adv;
   if (Cfg::EARLY_PARK) park_field_early<F>(D, out + (Cfg::E_OFF - Cfg::S_OFF) / 8, Cfg::THREADS);
 }
 
-// the field after which the RK-register tiles are asked for (they are needed only in the epilogue; asked for at kernel
-// start they queue ahead of the first ring refills)
-#ifndef Z4C_PQ_AT
-#define Z4C_PQ_AT 6
-#endif
 template <class Cfg, int IT>
 struct FieldLoop {
-  template <class LATE>
   __device__ __forceinline__ static void run(const CUtensorMap* map, unsigned char* tiles, uint64_t* full,
                                              const int toff, const int cx, const int cy, const int cz, const int b,
                                              const bool active, double* bw, double* aw, const FdConst& fd,
-                                             const SrcParams& sp, double* u, Derivs& D, double* out, LATE late) {
+                                             const SrcParams& sp, double* u, Derivs& D, double* out, double* scr,
+                                             const int ly, const int lz) {
     constexpr int S = IT % Cfg::NSTAGE;
     constexpr int F = stream_field(IT);
+    constexpr bool TWO = need_d2(F);
     // Every thread waits on the tile's barrier itself, right before it reads the tile. (Probing the barrier one field
     // ahead with mbarrier.test_wait and skipping this wait when the probe had already seen the phase complete was
     // measured: no faster, and on 256^3 runs a few cells per step read stale tile data -- DESIGN.md section 15.)
-    if (IT >= 3) mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);   // the first three were waited for up front
+    mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);
     const double* t = reinterpret_cast<const double*>(tiles + S * Cfg::STAGE_BYTES) + toff;
-    if (active) field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out);
-    if (IT + Cfg::NSTAGE < NF) {
-      __syncthreads();   // every thread is done reading stage S
-      if (threadIdx.x < 32) {
+    // the barrier after which nobody reads stage S (and, for a two-pass field, everybody has written its planes)
+    auto release = [&]() {
+      __syncthreads();
+      if (IT + Cfg::NSTAGE < NF && threadIdx.x < 32) {
         if (elect_one()) {
           mbar_expect_tx(&full[S], Cfg::TILE_BYTES);
           tma_load_5d(tiles + S * Cfg::STAGE_BYTES, map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
-          if (IT == Z4C_PQ_AT) late();
         }
       }
+    };
+    if (TWO) {
+      field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out, scr, ly, lz, release);
+    } else {
+      if (active) field_from_tile<Cfg, F>(t, bw, aw, fd, sp, u, D, out, scr, ly, lz, release);
+      // needed to free the ring slot, or because the next field rewrites the planes the previous one is still reading
+      constexpr bool NEXT_TWO = IT + 1 < NF && need_d2(stream_field(IT + 1 < NF ? IT + 1 : 0));
+      if (IT + Cfg::NSTAGE < NF || NEXT_TWO) release();
     }
-    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out, late);
+    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out, scr, ly, lz);
   }
 };
 template <class Cfg>
 struct FieldLoop<Cfg, NF> {
-  template <class LATE>
   __device__ __forceinline__ static void run(const CUtensorMap*, unsigned char*, uint64_t*, int, int, int, int, int,
                                              bool, double*, double*, const FdConst&, const SrcParams&, double*,
-                                             Derivs&, double*, LATE) {}
+                                             Derivs&, double*, double*, int, int) {}
 };
 
 // Arguments of the fused stage epilogue (STAGE 1..4): the RK registers, the OTHER state buffer (the stage
@@ -280,12 +345,16 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   const bool active = i < g.n && j < g.n && k < g.n;
   // gt^{ij} is needed while the very first fields stream in: the six centre values are requested before anything
   // else, so their latency overlaps the barrier set-up and the first tile copies
-  double gc[6];
+  // (the same for the shift, whose sign and size weight every field's advection)
+  double gc[6], bc[3];
   {
     const double* yc = sa.y_in + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG) + g.fs;
 #pragma unroll
     for (int p = 0; p < 6; ++p, yc += g.fs)   // one running pointer: gt_xx .. gt_zz are fields 1..6
       gc[p] = active ? __ldcg(yc) : (p == 0 || p == 3 || p == 5 ? 1.0 : 0.0);
+    yc += (long long)(BETAX - GZZ - 1) * g.fs;
+#pragma unroll
+    for (int a = 0; a < 3; ++a, yc += g.fs) bc[a] = active ? __ldcg(yc) : 0.0;
   }
   if (tid == 0) {
 #pragma unroll
@@ -356,8 +425,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   double bw[3], aw[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    mbar_wait(&full[a], 0);
-    const double beta = reinterpret_cast<const double*>(tiles + a * Cfg::STAGE_BYTES)[toff];
+    const double beta = bc[a];
     bw[a] = beta * (0.5 * fd.inv12h);
     aw[a] = fabs(beta) * (0.5 * fd.inv12h) + fd.ko;
   }
@@ -365,17 +433,21 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   double* park = reinterpret_cast<double*>(tiles + Cfg::S_OFF) + tid;
   Derivs D;
   derivs_begin(gc, D);
-  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park, [&]() {
-    // the RK registers of this tile, all 22 fields in one box each (run by the one elected thread)
-    if (STAGE >= 2 && Cfg::PQ_TMA) {
+  FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park,
+                         reinterpret_cast<double*>(tiles + Cfg::SCR_OFF), ly, lz);
+  double out[NF];
+  constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
+  static_assert(PARK || !Cfg::PQ_TMA, "the barrier below also frees the planes in the P/Q tile area");
+  if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring and with the planes
+  if (STAGE >= 2 && Cfg::PQ_TMA && tid < 32) {
+    // the RK registers of this tile, all 22 fields in one box each: asked for now that the planes of the two-pass
+    // derivatives no longer need the area; they land while the tensor algebra runs
+    if (elect_one()) {
       mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
       tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
       if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
     }
-  });
-  double out[NF];
-  constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
-  if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring
+  }
   if (active) {
 #pragma unroll
     for (int f = 0; f < NF; ++f) out[f] = 0.0;
