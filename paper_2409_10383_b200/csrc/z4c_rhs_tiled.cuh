@@ -87,7 +87,7 @@ struct TileCfg {
   static constexpr int PX_PLANE = PXY * TX, PX_ELEMS = PZ * PX_PLANE, PY_PLANE = TY * TX, PY_ELEMS = PZ * PY_PLANE;
   static constexpr int MIX_BYTES = ((PX_ELEMS + PY_ELEMS) * 8 + 127) / 128 * 128;
   static constexpr int SCR_OFF = PQ_TMA ? P_OFF : E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0);
-  static_assert(!PQ_TMA || MIX_BYTES <= 2 * REG_BYTES, "the planes fit the P/Q tile area");
+  static_assert(!PQ_TMA || MIX_BYTES <= REG_BYTES, "the planes fit the P tile area (the Q tile arrives during the stream)");
   static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0) + (PQ_TMA ? 0 : MIX_BYTES);   // push lists
   static constexpr int MAXLIST = 32;
   static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
@@ -263,13 +263,17 @@ __device__ __forceinline__ void field_from_tile(const double* t, const double* b
   if (Cfg::EARLY_PARK) park_field_early<F>(D, out + (Cfg::E_OFF - Cfg::S_OFF) / 8, Cfg::THREADS);
 }
 
+// the field at whose barrier the Q tile of the RK registers is asked for (it is needed only in the epilogue; asked for at
+// kernel start it queues ahead of the first ring refills)
+constexpr int Q_AT = 6;
 template <class Cfg, int IT>
 struct FieldLoop {
+  template <class EARLY>
   __device__ __forceinline__ static void run(const CUtensorMap* map, unsigned char* tiles, uint64_t* full,
                                              const int toff, const int cx, const int cy, const int cz, const int b,
                                              const bool active, double* bw, double* aw, const FdConst& fd,
                                              const SrcParams& sp, double* u, Derivs& D, double* out, double* scr,
-                                             const int ly, const int lz) {
+                                             const int ly, const int lz, EARLY early) {
     constexpr int S = IT % Cfg::NSTAGE;
     constexpr int F = stream_field(IT);
     constexpr bool TWO = need_d2(F);
@@ -285,6 +289,7 @@ struct FieldLoop {
         if (elect_one()) {
           mbar_expect_tx(&full[S], Cfg::TILE_BYTES);
           tma_load_5d(tiles + S * Cfg::STAGE_BYTES, map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
+          if (IT == Q_AT) early();
         }
       }
     };
@@ -296,14 +301,16 @@ struct FieldLoop {
       constexpr bool NEXT_TWO = IT + 1 < NF && need_d2(stream_field(IT + 1 < NF ? IT + 1 : 0));
       if (IT + Cfg::NSTAGE < NF || NEXT_TWO) release();
     }
-    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out, scr, ly, lz);
+    FieldLoop<Cfg, IT + 1>::run(map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, out, scr, ly, lz,
+                                early);
   }
 };
 template <class Cfg>
 struct FieldLoop<Cfg, NF> {
+  template <class EARLY>
   __device__ __forceinline__ static void run(const CUtensorMap*, unsigned char*, uint64_t*, int, int, int, int, int,
                                              bool, double*, double*, const FdConst&, const SrcParams&, double*,
-                                             Derivs&, double*, double*, int, int) {}
+                                             Derivs&, double*, double*, int, int, EARLY) {}
 };
 
 // Arguments of the fused stage epilogue (STAGE 1..4): the RK registers, the OTHER state buffer (the stage
@@ -359,7 +366,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < Cfg::NSTAGE; ++s) mbar_init(&full[s], 1);
-    mbar_init(pqbar, 1);
+    mbar_init(pqbar, STAGE >= 3 ? 2 : 1);   // one arrival per RK-register tile asked for (Q early, P late)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -434,18 +441,23 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   Derivs D;
   derivs_begin(gc, D);
   FieldLoop<Cfg, 0>::run(&map, tiles, full, toff, cx, cy, cz, b, active, bw, aw, fd, sp, u, D, park,
-                         reinterpret_cast<double*>(tiles + Cfg::SCR_OFF), ly, lz);
+                         reinterpret_cast<double*>(tiles + Cfg::SCR_OFF), ly, lz, [&]() {
+    // the Q tile of the RK registers, all 22 fields in one box (run by the one elected thread): its area is idle
+    if (STAGE >= 2 && Cfg::PQ_TMA) {
+      mbar_expect_tx(pqbar, Cfg::REG_BYTES);
+      tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
+    }
+  });
   double out[NF];
   constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
   static_assert(PARK || !Cfg::PQ_TMA, "the barrier below also frees the planes in the P/Q tile area");
   if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring and with the planes
-  if (STAGE >= 2 && Cfg::PQ_TMA && tid < 32) {
-    // the RK registers of this tile, all 22 fields in one box each: asked for now that the planes of the two-pass
-    // derivatives no longer need the area; they land while the tensor algebra runs
+  if (STAGE >= 3 && Cfg::PQ_TMA && tid < 32) {
+    // the P tile: asked for now that the planes of the two-pass derivatives no longer need its area; it lands while
+    // the tensor algebra runs
     if (elect_one()) {
-      mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
-      tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
-      if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
+      mbar_expect_tx(pqbar, Cfg::REG_BYTES);
+      tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
     }
   }
   if (active) {
