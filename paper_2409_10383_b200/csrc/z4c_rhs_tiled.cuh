@@ -69,7 +69,10 @@ struct TileCfg {
   static constexpr int TILE_ELEMS = HX * HY * HZ;
   static constexpr int TILE_BYTES = TILE_ELEMS * 8;
   static constexpr int STAGE_BYTES = (TILE_BYTES + 127) / 128 * 128;
-  static constexpr int BAR_OFF = NSTAGE * STAGE_BYTES;            // NSTAGE + 1 mbarriers
+  // With the RK-register tiles in shared memory a 4th ring slot lives in the Q tile's area, which is idle during the
+  // field stream (both register tiles are then asked for after the stream).
+  static constexpr int PHYS = (PQ_TMA_ && NSTAGE_ == 4) ? 3 : NSTAGE_;
+  static constexpr int BAR_OFF = PHYS * STAGE_BYTES;              // NSTAGE + 1 mbarriers
   static constexpr int REG_BYTES = NF * THREADS * 8;              // one RK-register tile [22][TZ][TY][TX]
   static constexpr int P_OFF = BAR_OFF + 128;                     // P tile, later the staged new state
   static constexpr int Q_OFF = P_OFF + (PQ_TMA ? REG_BYTES : 0);
@@ -90,6 +93,8 @@ struct TileCfg {
   static_assert(!PQ_TMA || MIX_BYTES <= REG_BYTES, "the planes fit the P tile area (the Q tile arrives during the stream)");
   static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0) + (PQ_TMA ? 0 : MIX_BYTES);   // push lists
   static constexpr int MAXLIST = 32;
+  __host__ __device__ static constexpr int slot_off(int s) { return s < PHYS ? s * STAGE_BYTES : Q_OFF; }
+  static_assert(PHYS == NSTAGE_ || STAGE_BYTES <= REG_BYTES, "the 4th slot fits the Q tile area");
   static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
   static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
   static_assert(TX + 2 * NG <= MAXLIST && TY + 2 * NG <= MAXLIST && TZ + 2 * NG <= MAXLIST, "push list size");
@@ -281,15 +286,15 @@ struct FieldLoop {
     // ahead with mbarrier.test_wait and skipping this wait when the probe had already seen the phase complete was
     // measured: no faster, and on 256^3 runs a few cells per step read stale tile data -- DESIGN.md section 15.)
     mbar_wait(&full[S], (IT / Cfg::NSTAGE) & 1);
-    const double* t = reinterpret_cast<const double*>(tiles + S * Cfg::STAGE_BYTES) + toff;
+    const double* t = reinterpret_cast<const double*>(tiles + Cfg::slot_off(S)) + toff;
     // the barrier after which nobody reads stage S (and, for a two-pass field, everybody has written its planes)
     auto release = [&]() {
       __syncthreads();
       if (IT + Cfg::NSTAGE < NF && threadIdx.x < 32) {
         if (elect_one()) {
           mbar_expect_tx(&full[S], Cfg::TILE_BYTES);
-          tma_load_5d(tiles + S * Cfg::STAGE_BYTES, map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
-          if (IT == Q_AT) early();
+          tma_load_5d(tiles + Cfg::slot_off(S), map, &full[S], cx, cy, cz, b, stream_field(IT + Cfg::NSTAGE));
+          if (IT == Q_AT && Cfg::PHYS == Cfg::NSTAGE) early();
         }
       }
     };
@@ -366,7 +371,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < Cfg::NSTAGE; ++s) mbar_init(&full[s], 1);
-    mbar_init(pqbar, STAGE >= 3 ? 2 : 1);   // one arrival per RK-register tile asked for (Q early, P late)
+    mbar_init(pqbar, (STAGE >= 3 && Cfg::PHYS == Cfg::NSTAGE) ? 2 : 1);   // one arrival per RK-register tile asked for (Q early, P late)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -374,7 +379,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 #pragma unroll
     for (int s = 0; s < Cfg::NSTAGE; ++s) {
       mbar_expect_tx(&full[s], Cfg::TILE_BYTES);
-      tma_load_5d(tiles + s * Cfg::STAGE_BYTES, &map, &full[s], cx, cy, cz, b, stream_field(s));
+      tma_load_5d(tiles + Cfg::slot_off(s), &map, &full[s], cx, cy, cz, b, stream_field(s));
     }
   }
   // push lists (O2): per axis, every (source cell of this tile -> destination block, padded index) pair, the
@@ -449,10 +454,18 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     }
   });
   double out[NF];
-  constexpr bool PARK = Cfg::NSTAGE * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
+  constexpr bool PARK = Cfg::PHYS * Cfg::STAGE_BYTES >= NPARK * Cfg::THREADS * 8;
   static_assert(PARK || !Cfg::PQ_TMA, "the barrier below also frees the planes in the P/Q tile area");
   if (PARK) __syncthreads();   // all threads (active or not) are done with the tile ring and with the planes
-  if (STAGE >= 3 && Cfg::PQ_TMA && tid < 32) {
+  if (Cfg::PHYS != Cfg::NSTAGE) {
+    if (STAGE >= 2 && Cfg::PQ_TMA && tid < 32) {   // both register tiles now: the 4th ring slot used the Q area
+      if (elect_one()) {
+        mbar_expect_tx(pqbar, (STAGE >= 3 ? 2 : 1) * Cfg::REG_BYTES);
+        tma_load_5d(sQ, &qmap, pqbar, cx, cy, cz, b, 0);
+        if (STAGE >= 3) tma_load_5d(sP, &pmap, pqbar, cx, cy, cz, b, 0);
+      }
+    }
+  } else if (STAGE >= 3 && Cfg::PQ_TMA && tid < 32) {
     // the P tile: asked for now that the planes of the two-pass derivatives no longer need its area; it lands while
     // the tensor algebra runs
     if (elect_one()) {
@@ -575,7 +588,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   8-wide tiles (8x4x4, 8x8x2: 20 % fewer halo bytes) are 20 % slower: 64-byte rows halve the coalescing of the
 //   register / state rows and put two tile rows of a warp on the same shared-memory banks.
 #if Z4C_NG == 3
-using RhsTile = TileCfg<16, 4, 2, 3, 2>;
+// 4-deep ring: three slots of their own, the 4th in the Q tile's area (+1.1 % on configs[3], +1.6 % on configs[1] over
+// the 3-deep ring with the Q tile asked for during the stream)
+using RhsTile = TileCfg<16, 4, 2, 4, 2>;
 #else
 // 4 ghosts: the halo tile grows to 24 x 12 x 10 (23 KB); to keep 2 CTAs per SM the P/Q tiles are read by batched
 // global loads instead of TMA (93 KB of shared memory per CTA)
