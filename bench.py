@@ -482,6 +482,117 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------
+# NEXT-3: two-level static refinement (the refined-box wave of PAPER.md:171 at bench size)
+# ------------------------------------------------------------------------------------------------
+TWO_LEVEL_LABEL = ("NEXT-3: linear wave, coarse 256^3 = 512 blocks of 32^3 (periodic), the 128^3 box at coarse cell "
+                   "(64,64,64) refined 2:1 into 256^3 fine cells = 512 blocks of 32^3; one dt, level exchange every stage")
+
+
+def two_level_workload(small: bool = False):
+    N, n = (32, 16) if small else (256, 32)
+    pc = replace(I.params_linear_wave(N, n), cfl=0.125)
+    pf = replace(pc, dx=pc.dx / 2, cfl=0.25, bc=1)                     # as many fine blocks as coarse blocks
+    origin = (N // 4,) * 3
+    pf = replace(pf, xmin=tuple(x + o * pc.dx for x, o in zip(pc.xmin, origin)))
+    return pc, pf, origin
+
+
+def run_two_level(args):
+    import torch
+    from paper_2409_10383_b200 import build, z4c
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the Z4c path has no CPU fallback")
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("the two-level workload runs on one GPU")
+    build.build()
+    pc, pf, origin = two_level_workload()
+    coarse = z4c.Z4c(pc, device="cuda:0")
+    fine = z4c.Z4c(pf, device="cuda:0", stream=coarse.stream)
+    for s in (coarse, fine):
+        s.set_fused(args.fuse)
+    coarse.set_initial_data(I.linear_wave_data(pc))
+    fine.set_initial_data(I.linear_wave_data(pf))
+    K, W, R = args.steps, max(args.warmup, 3), max(args.repeats, 1)
+    covered = (pf.N[0] // 2) * (pf.N[1] // 2) * (pf.N[2] // 2)
+    leaf = pc.ncells - covered + pf.ncells                                # zones of the leaf blocks
+
+    def timed(fn, reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(coarse.stream)
+        for _ in range(reps):
+            fn()
+        e1.record(coarse.stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    l0 = coarse.launch_count() + fine.launch_count()
+    fine.two_level_step(coarse, origin, W)
+    sampler = ClockSampler(0)
+    sampler.start()
+    times = [timed(lambda: fine.two_level_step(coarse, origin, K), 1) for _ in range(R)]
+    clocks = sampler.stop()
+    launches_per_step = (coarse.launch_count() + fine.launch_count() - l0) // (W + K * R)
+    ms = float(np.median(times))
+    # the pieces on their own: each level's RK4 step without the exchange, and the two exchange kernels
+    parts = {"coarse_step": timed(lambda: coarse.step(1), 5), "fine_step": timed(lambda: fine.step(1), 5),
+             "restrict_x4": 4 * timed(lambda: fine.restrict_to(coarse, origin), 20),
+             "prolongate_x4": 4 * timed(lambda: fine.prolongate_from(coarse, origin), 20)}
+    coarse.sync()
+    fine.sync()
+    eff = [list(coarse.effective_mode()), list(fine.effective_mode())]
+    # exchange kernels: algorithmic bytes = one read of every stencil node's 8 bytes once per output + the output
+    g, nn = pc.ng, pc.ng + 1
+    fine_ghost_out = 0
+    for bz in range(pf.nb[2]):
+        for by in range(pf.nb[1]):
+            for bx in range(pf.nb[0]):
+                ext = [pf.n + (g if b == 0 else 0) + (g if b == nb - 1 else 0) for b, nb in zip((bx, by, bz), pf.nb)]
+                fine_ghost_out += ext[0] * ext[1] * ext[2] - pf.n ** 3
+    hbm_peak, hbm_src = measured_peaks()
+    # restriction: every fine active cell read once, every covered coarse cell written; prolongation: every fine ghost
+    # cell outside the box written, ~0.4 coarse cells read per such cell (the layers of coarse nodes under the shell)
+    exch_bytes = 8 * I.NF * (pf.ncells + covered) + 8 * I.NF * int(1.4 * fine_ghost_out)
+    cpu = None
+    if not args.no_cpu:
+        from oracle import oracle as O
+        O.build()
+        qc, qf, qo = two_level_workload(small=True)
+        qf = replace(qf, nb=(1, 1, 1))
+        uc, uf = O.enforce(qc, I.linear_wave_data(qc))[0], O.enforce(qf, I.linear_wave_data(qf))[0]
+        t0 = time.perf_counter()
+        O.step_two_level(qc, qf, qf.n, qo, uc, uf, 1)
+        k = max(1, min(1000, int(10.0 / max(time.perf_counter() - t0, 1e-6))))
+        t0 = time.perf_counter()
+        O.step_two_level(qc, qf, qf.n, qo, uc, uf, k)
+        dt = time.perf_counter() - t0
+        qleaf = qc.ncells - qf.ncells // 8 + qf.ncells
+        cpu = {"value": qleaf * k / dt, "unit": "zone-cycles/s", "cores": O.num_threads(), "kind": "oracle",
+               "sample": f"coarse 32^3 in 8 blocks of 16^3 + one refined 16^3 block at coarse cell {qo}; {qleaf} leaf "
+                         f"zones x {k} two-level RK4 steps"}
+    line = {"metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": leaf * K / (ms * 1e-3), "unit": "zone-cycles/s",
+            "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": TWO_LEVEL_LABEL, "leaf_zones": leaf, "zones_computed": pc.ncells + pf.ncells,
+                       "note": "value counts the zones of leaf blocks only; the covered coarse cells are advanced too "
+                               "and then overwritten by the restriction",
+                       "effective_mode": eff, "l2": "no flush: working set of both packs exceeds the 126 MB L2"},
+            "repeats": {"n": R, "ms_per_step_each": [t / K for t in times], "statistic": "median"}, "clocks": clocks,
+            "gpu_launches": int(launches_per_step * K),
+            "two_level": {"ms_per_step_parts": parts,
+                          "exchange_share_of_step": 1.0 - (parts["coarse_step"] + parts["fine_step"]) / (ms / K),
+                          "exchange_roofline": {"bound": "hbm", "kernels": "k_restrict + k_prolong, 4 of each per step",
+                                                "achieved": 4 * exch_bytes / ((parts["restrict_x4"] + parts["prolongate_x4"]) * 1e-3) * 1e-9,
+                                                "peak": hbm_peak, "unit": "GB/s", "peak_source": hbm_src,
+                                                "bytes_per_exchange": exch_bytes}},
+            "cpu_baseline": cpu}
+    line["two_level"]["exchange_roofline"]["frac"] = line["two_level"]["exchange_roofline"]["achieved"] / hbm_peak
+    print(json.dumps(line))
+    coarse.close()
+    fine.close()
+
+
 def free_port() -> int:
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
@@ -512,6 +623,8 @@ def main():
         raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "two_level_wave_256":
+        run_two_level(args)
     else:
         run_ours(args)
 

@@ -126,16 +126,21 @@ int z4c_refine_indicators(z4c_ctx* ctx, double chi_min, double dchi_max, double*
  *
  * z4c_restrict: step 1 of MeshBlock B's protocol: every coarse interior cell covered by the fine box <-
  *   interpolation of the fine ACTIVE cells; the stencil is the n nearest fine nodes, shifted so that it never leaves
- *   the active region of the fine block that owns the cell's children. Then the coarse ghosts are
- *   refilled, which hands the new values to the coarse neighbours (steps A.2 / B.2). Async.
+ *   the active region of the fine block that owns the cell's children. The same kernel writes every
+ *   ghost image of the cells it restricts (wrap / clamp rule of O2), which hands the new values to the coarse
+ *   neighbours (steps A.2 / B.2): coarse ghosts that were current before the call are current after
+ *   it. Async.
  * z4c_prolongate: step 5: every ghost cell of the fine pack that lies outside the fine box (faces, edges
  *   and corners) <- interpolation of the n^3 nearest coarse nodes, read from the coarse INTERIOR cells through the
  *   coarse level's own wrap / clamp rule. Fine ghosts inside the box are the same-level exchange's. Async.
  * z4c_two_level_step: nsteps RK4 steps of both levels with one dt (no subcycling: coarse cfl*dx must equal fine
  *   cfl*dx); after every stage: stage update with same-level ghost push on both packs, z4c_restrict, z4c_prolongate
  *   (and once on entry, so the levels are consistent whatever the caller loaded). The set-up of the paper's
- *   refined-corner wave test. Runs the unfused launch sequence (RHS, update + push per level). Async.
- * Errors: Z4C_EINVAL (different streams, spacing not 2:1, box outside the coarse mesh, odd n, unequal dt). */
+ *   refined-corner wave test. With both contexts in mode 2 (z4c_set_fused) every stage is the fused
+ *   stage kernel on each level followed by the two exchange kernels on the buffer just written (4 launches per stage);
+ *   otherwise RHS, update + push per level, then the exchange (6 launches per stage). Async.
+ * Errors: Z4C_EINVAL (different streams, spacing not 2:1, box outside the coarse mesh, odd n, unequal dt, a
+ *   partitioned pack). */
 int z4c_restrict(z4c_ctx* fine, z4c_ctx* coarse, const int32_t* origin);
 int z4c_prolongate(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin);
 int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, int nsteps);

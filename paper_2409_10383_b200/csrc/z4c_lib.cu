@@ -121,9 +121,9 @@ int grid_for(long long total, int threads, long long cap = (1LL << 30)) {
 }
 
 // ---- launch helpers (all asynchronous on c->stream) ---------------------------------------
-int launch_ghost_fill(z4c_ctx* c) {
+int launch_ghost_fill(z4c_ctx* c, int buf = 0) {
   const long long per_block = 2LL * NG * ((long long)c->g.m * c->g.m + (long long)c->g.n * c->g.m + (long long)c->g.n * c->g.n);
-  k_ghost_fill<<<grid_for(per_block * c->g.nblk, 256), 256, 0, c->stream>>>(c->g, c->y, make_slab(c, 0));
+  k_ghost_fill<<<grid_for(per_block * c->g.nblk, 256), 256, 0, c->stream>>>(c->g, c->ybuf[buf], make_slab(c, buf));
   return check_launch(c, "k_ghost_fill");
 }
 
@@ -538,6 +538,7 @@ namespace {
 int check_levels(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, AmrGeom* a) {
   if (!coarse || !fine || !origin || coarse == fine) return Z4C_EINVAL;
   if (coarse->stream != fine->stream) return fail(fine, Z4C_EINVAL, "two-level calls need both contexts on one stream");
+  if (partitioned(coarse) || partitioned(fine)) return fail(fine, Z4C_EINVAL, "two-level calls need unpartitioned packs");
   if (fine->g.n % 2) return fail(fine, Z4C_EINVAL, "restriction needs an even block size");
   if (std::fabs(2.0 * fine->prm.dx - coarse->prm.dx) > 1e-12 * coarse->prm.dx)
     return fail(fine, Z4C_EINVAL, "fine dx must be half the coarse dx");
@@ -549,24 +550,24 @@ int check_levels(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, AmrGeom*
   }
   return Z4C_OK;
 }
-int launch_restrict(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a) {
+int launch_restrict(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
   const long long total = (long long)a.Mc[0] * a.Mc[1] * a.Mc[2] * NF;
-  k_restrict<<<grid_for(total, 128), 128, 0, fine->stream>>>(fine->g, fine->y, coarse->g, coarse->y, a);
+  k_restrict<<<grid_for(total, 128), 128, 0, fine->stream>>>(fine->g, fine->ybuf[buf], coarse->g, coarse->ybuf[buf], a,
+                                                                  make_amr_weights(fine->g.n));
   return check_launch(fine, "k_restrict");
 }
-int launch_prolong(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a) {
+int launch_prolong(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
   const Pack& g = fine->g;
-  const long long per_block = 2LL * NG * ((long long)g.m * g.m + (long long)g.n * g.m + (long long)g.n * g.n);
-  k_prolong<<<grid_for(per_block * g.nblk * NF, 128), 128, 0, fine->stream>>>(coarse->g, coarse->y, g, fine->y, a);
+  k_prolong<<<grid_for(prolong_shell_cells(g.n, g.nb), 128), 128, 0, fine->stream>>>(coarse->g, coarse->ybuf[buf], g,
+                                                                               fine->ybuf[buf], a,
+                                                                               make_amr_weights(g.n));
   return check_launch(fine, "k_prolong");
 }
-// steps B.1, A.2/B.2 (the covered coarse nodes reach the coarse neighbours through the same-level fill), B.5
-int sync_levels(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a) {
-  int rc = launch_restrict(coarse, fine, a);
+// steps B.1, A.2/B.2 (k_restrict writes the ghost images of the covered coarse nodes itself), B.5; on state buffer `buf`
+int sync_levels(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
+  int rc = launch_restrict(coarse, fine, a, buf);
   if (rc) return rc;
-  rc = launch_ghost_fill(coarse);
-  if (rc) return rc;
-  return launch_prolong(coarse, fine, a);
+  return launch_prolong(coarse, fine, a, buf);
 }
 }  // namespace
 
@@ -574,9 +575,7 @@ int z4c_restrict(z4c_ctx* fine, z4c_ctx* coarse, const int32_t* origin) {
   AmrGeom a;
   int rc = check_levels(coarse, fine, origin, &a);
   if (rc) return rc;
-  rc = launch_restrict(coarse, fine, a);
-  if (rc) return rc;
-  return launch_ghost_fill(coarse);
+  return launch_restrict(coarse, fine, a);
 }
 
 int z4c_prolongate(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin) {
@@ -595,12 +594,21 @@ int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, in
   if (std::fabs(coarse->dt - fine->dt) > 1e-14 * fine->dt)
     return fail(fine, Z4C_EINVAL, "both levels advance with one dt (no subcycling): set cfl so that cfl*dx agrees");
   rc = sync_levels(coarse, fine, a);
+  // Both levels in mode 2: one stage kernel per level and stage (state ping-pong ybuf[in] -> ybuf[1 - in], ghost images
+  // written by the kernel), then the level exchange on the buffer just written. Otherwise K2 + K3-with-push in place.
+  const bool fused = fully_fused(coarse) && fully_fused(fine);
+  z4c_ctx* lv[2] = {coarse, fine};
   for (int st = 0; st < nsteps && rc == Z4C_OK; ++st)
     for (int s = 1; s <= 4 && rc == Z4C_OK; ++s) {
-      z4c_ctx* lv[2] = {coarse, fine};
-      for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_rhs(lv[q], coef[s - 1], lv[q]->dt);
-      for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_stage_update(lv[q], s, true);
-      if (rc == Z4C_OK) rc = sync_levels(coarse, fine, a);
+      const int in = (s - 1) & 1;
+      if (fused) {
+        for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_fused_stage(lv[q], s, in);
+        if (rc == Z4C_OK) rc = sync_levels(coarse, fine, a, 1 - in);
+      } else {
+        for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_rhs(lv[q], coef[s - 1], lv[q]->dt);
+        for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_stage_update(lv[q], s, true);
+        if (rc == Z4C_OK) rc = sync_levels(coarse, fine, a);
+      }
     }
   if (rc == Z4C_OK) { coarse->steps += nsteps; fine->steps += nsteps; }
   return rc;

@@ -92,13 +92,18 @@ def test_restrict_and_prolongate_against_the_oracle(Z, oracle, name):
     fine.close()
 
 
-def test_two_level_steps_against_the_oracle(Z, oracle):
+@pytest.mark.parametrize("mode", [2, 1])
+def test_two_level_steps_against_the_oracle(Z, oracle, mode):
     """The refined-corner wave of PAPER.md:171 on BASELINE's wave: coarse 32^3 in 8 blocks of 16^3, the corner block
-    refined once (8 fine blocks of 16^3), one dt; 1 step at 1e-12, 12 steps at 1e-10, both levels."""
+    refined once (8 fine blocks of 16^3), one dt; 1 step at 1e-12, 12 steps at 1e-10, both levels. mode 2: the fused
+    stage kernel per level and stage (state ping-pong), mode 1: RHS + update-with-push in place."""
     pc = replace(I.params_linear_wave(32, 16), cfl=0.125)
     pf = replace(pc, nb=(2, 2, 2), dx=pc.dx / 2, cfl=0.25, bc=1)
     uc, uf = I.linear_wave_data(pc), I.linear_wave_data(pf)
     coarse, fine = levels(Z, pc, pf, uc, uf)
+    for s in (coarse, fine):
+        s.set_fused(mode)
+        assert s.effective_mode()[1] == mode
     rc, rf = oracle.enforce(pc, uc)[0], oracle.enforce(pf, uf)[0]
     done = 0
     for target, tol in ((1, 1e-12), (12, 1e-10)):
@@ -119,6 +124,8 @@ def test_two_level_steps_against_the_oracle(Z, oracle):
     # fine data = the coarse field interpolated onto the fine box (by the oracle), so the levels start consistent
     u2f = oracle.prolong(oracle.enforce(pc2, u2c)[0], 3, pc2.bc, o, (0, 0, 0), pf2.N)
     c2, f2 = levels(Z, pc2, pf2, u2c, u2f)
+    for s in (c2, f2):
+        s.set_fused(mode)
     rc2, rf2, bad = oracle.step_two_level(pc2, pf2, 8, o, oracle.enforce(pc2, u2c)[0], oracle.enforce(pf2, u2f)[0], 1)
     assert bad == 0
     f2.two_level_step(c2, o, 1)
