@@ -96,14 +96,17 @@ struct AmrGeom {
 // for those cells: the thread also writes the ghost images of its coarse cell (same wrap / clamp rule as O2, the
 // target list of the stage update's push), so the coarse level needs no whole-pack ghost fill after a restriction.
 // One thread per (covered coarse cell, field).
-__global__ void __launch_bounds__(128) k_restrict(Pack gf, const double* __restrict__ yf, Pack gc,
+constexpr int RB_X = 16, RB_Y = 4, RB_Z = 2;   // k_restrict's brick of coarse cells per CTA (128 threads)
+__global__ void __launch_bounds__(RB_X * RB_Y * RB_Z) k_restrict(Pack gf, const double* __restrict__ yf, Pack gc,
                                                   double* __restrict__ yc, AmrGeom a, AmrWeights wt) {
-  const long long ncov = (long long)a.Mc[0] * a.Mc[1] * a.Mc[2];
-  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (t >= ncov * NF) return;
-  const int f = (int)(t / ncov);
-  const long long c = t - f * ncov;
-  const int C[3] = {(int)(c % a.Mc[0]), (int)((c / a.Mc[0]) % a.Mc[1]), (int)(c / ((long long)a.Mc[0] * a.Mc[1]))};
+  // a CTA takes a 16 x 4 x 2 brick of coarse cells of one field, so that the fine rows and planes its threads share
+  // (half of each stencil overlaps the neighbour's) are found in this SM's L1
+  const int bricks_x = (a.Mc[0] + RB_X - 1) / RB_X, bricks_y = (a.Mc[1] + RB_Y - 1) / RB_Y;
+  const int f = blockIdx.y;
+  const int bx = blockIdx.x % bricks_x, by = (blockIdx.x / bricks_x) % bricks_y, bz = blockIdx.x / (bricks_x * bricks_y);
+  const int C[3] = {bx * RB_X + (int)(threadIdx.x % RB_X), by * RB_Y + (int)((threadIdx.x / RB_X) % RB_Y),
+                    bz * RB_Z + (int)(threadIdx.x / (RB_X * RB_Y))};
+  if (C[0] >= a.Mc[0] || C[1] >= a.Mc[1] || C[2] >= a.Mc[2]) return;
   double w[3][AMR_N];
   int s[3], fb[3], ref[3];
   const int half = gf.n / 2;
@@ -201,7 +204,8 @@ __global__ void __launch_bounds__(128) k_prolong(Pack gc, const double* __restri
     gi[0] = q < NG ? q - NG : Nx + q - NG; gi[1] = (int)((r / G2) % Ny); gi[2] = (int)(r / ((long long)G2 * Ny));
   }
   double w[3][AMR_N];
-  long long off[3][AMR_N];   // per axis: offset contribution of every stencil node inside the coarse pack
+  int off[3][AMR_N];         // per axis: offset contribution of every stencil node inside one field of the coarse pack
+                             // (32 bits: the launcher refuses a coarse field of 2^31 doubles or more)
   int ref[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
@@ -214,10 +218,10 @@ __global__ void __launch_bounds__(128) k_prolong(Pack gc, const double* __restri
       int G = s + q;
       if (gc.bc == 0) { G %= N; if (G < 0) G += N; } else { G = G < 0 ? 0 : (G >= N ? N - 1 : G); }
       const int cb = G / gc.n;
-      off[d][q] = cb * bstride + (long long)(G - cb * gc.n + NG) * lstride;
+      off[d][q] = (int)(cb * bstride + (long long)(G - cb * gc.n + NG) * lstride);
     }
   }
-  long long roff = 0;
+  int roff = 0;
 #pragma unroll
   for (int q = 0; q < AMR_N; ++q)          // ref[] is a run-time index: select instead of indexing the register array
     if (q == ref[2])

@@ -551,13 +551,16 @@ int check_levels(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, AmrGeom*
   return Z4C_OK;
 }
 int launch_restrict(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
-  const long long total = (long long)a.Mc[0] * a.Mc[1] * a.Mc[2] * NF;
-  k_restrict<<<grid_for(total, 128), 128, 0, fine->stream>>>(fine->g, fine->ybuf[buf], coarse->g, coarse->ybuf[buf], a,
-                                                                  make_amr_weights(fine->g.n));
+  const long long bricks = (long long)((a.Mc[0] + RB_X - 1) / RB_X) * ((a.Mc[1] + RB_Y - 1) / RB_Y) *
+                           ((a.Mc[2] + RB_Z - 1) / RB_Z);
+  if (bricks > 0x7fffffffLL) return fail(fine, Z4C_EINVAL, "fine region too large for one k_restrict launch");
+  k_restrict<<<dim3((unsigned)bricks, NF), RB_X * RB_Y * RB_Z, 0, fine->stream>>>(
+      fine->g, fine->ybuf[buf], coarse->g, coarse->ybuf[buf], a, make_amr_weights(fine->g.n));
   return check_launch(fine, "k_restrict");
 }
 int launch_prolong(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
   const Pack& g = fine->g;
+  if (coarse->g.fs > 0x7fffffffLL) return fail(fine, Z4C_EINVAL, "coarse pack too large for k_prolong's 32-bit offsets");
   k_prolong<<<grid_for(prolong_shell_cells(g.n, g.nb), 128), 128, 0, fine->stream>>>(coarse->g, coarse->ybuf[buf], g,
                                                                                fine->ybuf[buf], a,
                                                                                make_amr_weights(g.n));
