@@ -109,6 +109,27 @@ int z4c_step(z4c_ctx* ctx, int nsteps);
  * Returns Z4C_ESTATE if the device error flag is set. */
 int z4c_constraints(z4c_ctx* ctx, double* out, double* d_percell);
 
+/* The same eight norms WITHOUT touching any allocator and without synchronising: for callers that cannot allocate or
+ * block (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc). Inputs: the context's
+ * current state (ghosts valid). Output: d_out, DEVICE pointer to 8 doubles, same order as z4c_constraints, written
+ * by the second of two kernels enqueued on the context's stream (asynchronous; no device error-flag read).
+ * Scratch: one row of 8 partial norms per MeshBlock in a file-scope `static __device__` array of the library,
+ * Z4C_STATIC_MAX_BLOCKS = 4096 rows = 256 KiB, which every GPU that loads the library holds until the process exits.
+ * Its device address is looked up with cudaGetSymbolAddress on the first call on each device (the context's device
+ * must be current, as for every call): make that first call outside graph capture. The call uses no cudaMalloc,
+ * cudaFree or other allocating routine, and no part of the caller's workspace.
+ * Limit: packs of more than 4096 MeshBlocks are refused with Z4C_EINVAL and a message (z4c_last_error); use
+ * z4c_constraints for those.
+ * Sharing: ALL calls on a device, from every context and stream, use the same array. It keeps the last call's rows;
+ * every row a call reads it has written first (one CTA per MeshBlock writes its row unconditionally), so nothing has to
+ * be cleared between calls. Two calls that OVERLAP on the GPU (different streams, or graphs replayed concurrently)
+ * race on the rows and return garbage: order them on one stream or with events.
+ * Numerics: the sums of squares are taken per MeshBlock and then over MeshBlocks in a fixed order (bitwise
+ * reproducible from call to call); z4c_constraints groups the same terms differently, so the rms values agree with
+ * it to rounding (a few ulp), the max values exactly. */
+#define Z4C_STATIC_MAX_BLOCKS 4096
+int z4c_constraints_static(z4c_ctx* ctx, double* d_out);
+
 /* AMR refinement indicators per MeshBlock (sections 3.3.1-3.3.2; no regridding here): for every
  * block b, d_minchi[b] = min of chi and d_maxdchi[b] = max of |grad chi| (Euclidean norm of the scheme's centred first
  * derivative) over the block's interior cells, d_flags[b] = (min chi < chi_min ? 1 : 0) | (max |grad chi| > dchi_max ?

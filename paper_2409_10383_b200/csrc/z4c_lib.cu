@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <mutex>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -278,6 +279,70 @@ int read_flag(z4c_ctx* c) {
   return Z4C_OK;
 }
 
+}  // namespace
+
+// ---- constraint monitors without any allocation (z4c_constraints_static, include/z4c.h) ---------------------------
+// For callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).
+// The scratch of the two-pass reduction -- one row of 8 partial norms per MeshBlock -- lives in a file-scope device
+// array of a fixed, modest size instead of the caller's workspace: 4096 rows x 8 doubles = 256 KiB, held by every GPU
+// that loads this library until the process exits. In HOST code the array's name is only a stand-in for the symbol:
+// the device address is looked up once per device with cudaGetSymbolAddress (static_scratch_ptr below) and handed to
+// the kernels as an ordinary pointer. All calls on a device share the array; it keeps the last call's rows.
+static __device__ __align__(256) double g_static_partial[(size_t)Z4C_STATIC_MAX_BLOCKS * 8];
+
+namespace z4c {
+// K4 with one CTA per MeshBlock: row b of `partial` <- {sum H^2, max|H|, sum |M|^2, max|M|, sum Theta^2, max|Theta|,
+// sum |Z|^2, max|Z|} over the interior cells of block b (same point function and per-CTA reduction as k_constraints).
+// Every row in [0, N_b) is written by its CTA on every call, so nothing in the scratch has to start at zero.
+__global__ void __launch_bounds__(K4_THREADS)
+    k_constraints_blocks(Pack g, const double* __restrict__ y, FdConst fd, SrcParams sp, double* __restrict__ partial) {
+  __shared__ double red[8 * (K4_THREADS / 32)];
+  double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const int b = blockIdx.x;
+  for (int r = threadIdx.x; r < g.n3; r += K4_THREADS) {
+    const int i = r % g.n, j = (r / g.n) % g.n, k = r / (g.n * g.n);
+    const double* yc = y + (long long)b * g.m3 + ((long long)(k + NG) * g.m + (j + NG)) * g.m + (i + NG);
+    double u[NF], out[NF], c[6];
+    Derivs D;
+    gather_global<false>(yc, g.fs, g.m, g.m2, fd, sp, u, D, out);
+    const int st[3] = {1, g.m, g.m2};
+    z4c_constraints_point(u, D, [&](const int a, double* q) {
+#pragma unroll
+      for (int p = 0; p < 6; ++p) q[p] = d1_raw(yc + (AXX + p) * g.fs, st[a]) * fd.inv12h;
+    }, c);
+    acc[0] += c[0] * c[0];          acc[1] = fmax(acc[1], fabs(c[0]));
+    acc[2] += c[4];                 acc[3] = fmax(acc[3], sqrt(c[4]));
+    acc[4] += u[THETA] * u[THETA];  acc[5] = fmax(acc[5], fabs(u[THETA]));
+    acc[6] += c[5];                 acc[7] = fmax(acc[7], sqrt(c[5]));
+  }
+  block_reduce8(acc, red);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) partial[(long long)b * 8 + q] = acc[q];
+  }
+}
+}  // namespace z4c
+
+namespace {
+// Device address of g_static_partial on the CURRENT device: looked up once per device, return code checked.
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+double* g_static_ptr[STATIC_MAX_DEVICES] = {};
+cudaError_t static_scratch_ptr(double** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_static_partial);
+    if (e != cudaSuccess) return e;
+    g_static_ptr[dev] = p;
+  }
+  *out = g_static_ptr[dev];
+  return cudaSuccess;
+}
 }  // namespace
 
 extern "C" {
@@ -685,6 +750,22 @@ int z4c_constraints_raw(z4c_ctx* c, double* out) {
                   "D2H copy");
   if (rc) return rc;
   return read_flag(c);
+}
+
+int z4c_constraints_static(z4c_ctx* c, double* d_out) {
+  if (!c || !d_out) return Z4C_EINVAL;
+  if (c->g.nblk > Z4C_STATIC_MAX_BLOCKS)
+    return fail(c, Z4C_EINVAL, "z4c_constraints_static: the pack has " + std::to_string(c->g.nblk) +
+                               " MeshBlocks, the static scratch holds " + std::to_string(Z4C_STATIC_MAX_BLOCKS) +
+                               " rows (use z4c_constraints, whose partials live in the caller's workspace)");
+  double* scratch = nullptr;
+  int rc = check_cuda(c, static_scratch_ptr(&scratch), "cudaGetSymbolAddress(static scratch)");
+  if (rc) return rc;
+  k_constraints_blocks<<<c->g.nblk, K4_THREADS, 0, c->stream>>>(c->g, c->y, c->fd, c->sp, scratch);
+  rc = check_launch(c, "k_constraints_blocks");
+  if (rc) return rc;
+  k_constraints_final<<<1, K4_THREADS, 0, c->stream>>>(scratch, c->g.nblk, (double)c->g.ncell, d_out);
+  return check_launch(c, "k_constraints_final");
 }
 
 int z4c_sync(z4c_ctx* c) {

@@ -20,7 +20,7 @@ LIB_PATH_NG4 = os.path.join(_HERE, "libz4c_ng4.so")    # built with 4 ghost zone
 
 # every symbol include/z4c.h declares
 SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_initial_data", "z4c_step",
-           "z4c_constraints", "z4c_refine_indicators", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
+           "z4c_constraints", "z4c_constraints_static", "z4c_refine_indicators", "z4c_get_interior", "z4c_fill_ghosts", "z4c_eval_rhs", "z4c_enforce", "z4c_sync",
            "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
            "z4c_probe_fp64", "z4c_effective_mode", "z4c_time",
            "z4c_restrict", "z4c_prolongate", "z4c_two_level_step",
@@ -76,6 +76,7 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_set_initial_data.argtypes = [vp, dp, C.c_int]
     L.z4c_step.argtypes = [vp, C.c_int]
     L.z4c_constraints.argtypes = [vp, C.POINTER(C.c_double), dp]
+    L.z4c_constraints_static.argtypes = [vp, dp]
     L.z4c_refine_indicators.argtypes = [vp, C.c_double, C.c_double, dp, dp, dp]
     L.z4c_get_interior.argtypes = [vp, dp, C.c_int]
     L.z4c_fill_ghosts.argtypes = [vp]
@@ -215,6 +216,16 @@ class Z4c:
             self._check(self.lib.z4c_constraints(self.h, out, pc.data_ptr() if percell else None))   # synchronises
         res = np.array(list(out))
         return (res, pc.cpu().numpy()) if percell else res
+
+    def constraints_static(self, d_out=None):
+        """z4c_constraints_static: the 8 norms into a DEVICE tensor (8 doubles; the caller's, or a new one), computed
+        with the library's static scratch: no allocation inside the call, asynchronous on the context's stream."""
+        if d_out is None:
+            d_out = self.torch.empty(8, dtype=self.torch.float64, device=self.device)
+            self._before(d_out)
+        with self.torch.cuda.device(self.device):
+            self._check(self.lib.z4c_constraints_static(self.h, d_out.data_ptr()))
+        return d_out
 
     def refine_indicators(self, chi_min: float, dchi_max: float):
         """z4c_refine_indicators: (min chi, max |grad chi|, flags) per block as numpy arrays."""
