@@ -173,3 +173,71 @@ def test_two_level_step_with_four_ghosts(Z, oracle):
         assert err.max() <= 1e-12, dict(zip(I.FIELD_NAMES, err))
     coarse.close()
     fine.close()
+
+
+def _padded_box_from_interior(u, p, b3):
+    """Padded box [F][m][m][m] of block b3 = (bx, by, bz) by O2's definition (periodic wrap) from the global interior."""
+    n, g = p.n, p.ng
+    idx = [(np.arange(-g, n + g) + b * n) % N for b, N in zip(b3, p.N)]
+    return u[:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]]
+
+
+def test_two_level_bench_workload_at_full_size(Z, oracle):
+    """The workload `bench.py --workload two_level_wave_256` times, in its launch configuration (both packs in mode 2:
+    fused stage kernel per level, exchange on the buffer just written; 512 + 512 blocks of 32^3), after two steps, on
+    sampled outputs the oracle computes one by one -- all bit for bit, since the exchange is bit-specified (R-I1):
+    covered coarse cells = oracle restriction of the fine blocks above them; coarse ghosts = images of the interior
+    (written by k_restrict for the cells it changed); fine ghosts outside the box = oracle prolongation of the coarse
+    interior (faces, edges, corners of the box); fine ghosts inside the box = the neighbouring fine block's cells.
+    Seeded 1e-10 noise on top of the x-directed wave makes every cell distinct, so a wrong y / z index cannot hide."""
+    import bench
+    import torch
+    pc, pf, origin = bench.two_level_workload()
+    uc0 = I.linear_wave_data(pc) + I.noise_data(pc, 31)
+    uf0 = I.linear_wave_data(pf) + I.noise_data(pf, 32)
+    coarse, fine = levels(Z, pc, pf, uc0, uf0)
+    del uc0, uf0
+    assert coarse.effective_mode()[1] == 2 and fine.effective_mode()[1] == 2
+    fine.two_level_step(coarse, origin, 2)
+    coarse.sync()
+    uc, uf = coarse.get_interior(), fine.get_interior()
+    assert np.all(np.isfinite(uc)) and np.all(np.isfinite(uf))
+    n, g, h = pc.n, pc.ng, pc.n // 2
+    # (i) restriction: coarse cells under sampled fine blocks (corner, far corner, inside, on a face of the box)
+    for bx, by, bz in ((0, 0, 0), (7, 7, 7), (3, 4, 5), (7, 0, 3)):
+        sub = uf[:, bz * n:(bz + 1) * n, by * n:(by + 1) * n, bx * n:(bx + 1) * n]
+        want = oracle.restrict(sub, g, n)
+        got = uc[:, origin[2] + bz * h:origin[2] + (bz + 1) * h, origin[1] + by * h:origin[1] + (by + 1) * h,
+                 origin[0] + bx * h:origin[0] + (bx + 1) * h]
+        assert np.array_equal(got, want), (bx, by, bz)
+    # (ii) coarse ghosts, blocks next to / inside / far from the box and across the periodic faces
+    for b3 in ((1, 2, 2), (2, 2, 2), (5, 6, 1), (0, 0, 0), (7, 7, 7), (4, 4, 4)):
+        b = (b3[2] * pc.nb[1] + b3[1]) * pc.nb[0] + b3[0]
+        assert np.array_equal(coarse.state[:, b].cpu().numpy(), _padded_box_from_interior(uc, pc, b3)), b3
+    # (iii) prolongation: windows of the shell around the fine region (indices relative to its corner)
+    Nf = pf.N[0]
+    windows = (((-g, 100, 100), (0, 140, 140)), ((Nf, 30, 200), (Nf + g, 70, 256)), ((90, -g, 10), (130, 0, 40)),
+               ((10, Nf, 10), (60, Nf + g, 40)), ((120, 120, -g), (136, 136, 0)), ((0, 224, Nf), (40, 256, Nf + g)),
+               ((-g, -g, -g), (0, 0, 0)), ((Nf, Nf, Nf), (Nf + g, Nf + g, Nf + g)), ((Nf, -g, 60), (Nf + g, 0, 68)),
+               ((-g, 28, Nf), (0, 36, Nf + g)))
+    state_f = fine.state
+    for lo, hi in windows:
+        want = oracle.prolong(uc, g, pc.bc, origin, lo, hi)
+        ax = []
+        for d in range(3):                                   # a block whose padded box holds each index, and where
+            c = np.arange(lo[d], hi[d])
+            bd = np.clip(c // n, 0, pf.nb[d] - 1)
+            ax.append((bd, c - bd * n + g))
+        (bxs, lxs), (bys, lys), (bzs, lzs) = ax
+        blk = (bzs[:, None, None] * pf.nb[1] + bys[None, :, None]) * pf.nb[0] + bxs[None, None, :]
+        got = state_f[:, torch.from_numpy(blk).to(state_f.device),
+                      torch.from_numpy(np.broadcast_to(lzs[:, None, None], blk.shape).copy()).to(state_f.device),
+                      torch.from_numpy(np.broadcast_to(lys[None, :, None], blk.shape).copy()).to(state_f.device),
+                      torch.from_numpy(np.broadcast_to(lxs[None, None, :], blk.shape).copy()).to(state_f.device)]
+        assert np.array_equal(got.cpu().numpy(), want), (lo, hi)
+    # (iv) fine ghosts inside the box: an inner block's padded box is a window of the fine interior
+    for b3 in ((3, 4, 5), (1, 1, 6)):
+        b = (b3[2] * pf.nb[1] + b3[1]) * pf.nb[0] + b3[0]
+        assert np.array_equal(state_f[:, b].cpu().numpy(), _padded_box_from_interior(uf, pf, b3)), b3
+    coarse.close()
+    fine.close()
