@@ -390,7 +390,17 @@ def run_ours(args):
         sim.step_timed(2)
         kt = sim.step_timed(Kt)
     total_kt = kt["rhs"] + kt["update"] + kt["ghost"]
-    fp64_peak = (sim.sim if partitioned else sim).probe_fp64()
+    core0 = sim.sim if partitioned else sim
+    fp64_burst = core0.probe_fp64()
+    # the same DFMA loop held for ~3 s with the clocks sampled: what the FP64 pipe sustains under the power cap that
+    # also holds the long timed region above (context for `frac`, which stays against the burst figure)
+    sus_sampler, sus_vals, t_sus = ClockSampler(local_rank), [], time.perf_counter()
+    sus_sampler.start()
+    while time.perf_counter() - t_sus < 3.0:
+        sus_vals.append(core0.probe_fp64(iters=2_000_000))
+    sus_clocks = sus_sampler.stop()
+    fp64_sustained = float(np.median(sus_vals[len(sus_vals) // 2:]))
+    fp64_peak = max(fp64_burst, fp64_sustained)      # the short probe right after the long run can catch a depressed clock
     hbm_peak, hbm_src = measured_peaks()
     flops_cell = RHS_FLOPS_PER_CELL if p.ng == 3 else RHS_FLOPS_PER_CELL_O6
     # dominant kernel = the RHS / fused stage kernel, 4 launches per step; its launch time from the graph-replayed
@@ -465,7 +475,14 @@ def run_ours(args):
                          "traffic": prof.get("mean_bytes_per_launch") if prof else None,
                          "traffic_commit": prof.get("commit") if prof else None,
                          "fp64_pipe_active_pct_ncu": prof.get("fp64_pipe_active_pct") if prof else None,
-                         "peak_source": "measured live: z4c_probe_fp64 DFMA loop (nominal %.1f at 1965 MHz)" % FP64_NOMINAL_TFLOPS,
+                         "peak_source": "measured live: z4c_probe_fp64 DFMA loop, the higher of a 3 ms burst and a 3 s run "
+                                        "(nominal %.1f at 1965 MHz)" % FP64_NOMINAL_TFLOPS,
+                         "peak_burst": fp64_burst,
+                         "peak_sustained": {"value": fp64_sustained, "unit": "TFLOP/s", "clocks": sus_clocks,
+                                            "what": "the same DFMA loop held for 3 s (median of the second half)"},
+                         "frac_of_sustained_peak": rhs_tflops / fp64_sustained,
+                         "frac_at_measured_clock": (rhs_tflops / (FP64_NOMINAL_TFLOPS * clocks["sm_mhz"] / 1965.0)
+                                                    if clocks and clocks.get("sm_mhz") else None),
                          "flops_per_cell": flops_cell, "ms_per_launch": rhs_ms,
                          "timing": "graph-replayed step / 4" if eff_fused == 2 else "events between kernels",
                          "share_of_step": kt["rhs"] / total_kt},

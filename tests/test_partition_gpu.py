@@ -74,6 +74,37 @@ def test_slabs_reproduce_the_single_pack_bitwise(Z, oracle, name, mode):
     many.close()
 
 
+def test_config3_in_four_slabs_at_full_size_bitwise(Z):
+    """BASELINE configs[3] (two punctures, 512 blocks of 32^3, outflow) as `bench.py --gpus 4` would cut it -- four
+    z-slabs of 2 block layers, mode 2, one stage kernel per slab and stage writing ghost images into the neighbouring
+    slabs' buffers -- against the single pack after 2 steps: padded states (interior and every ghost) bit for bit,
+    compared on the device."""
+    import torch
+    import bench
+    from paper_2409_10383_b200 import partition as PT
+    p, u, _ = bench.workload("bbh_256")
+    one = Z.Z4c(p)
+    one.set_initial_data(u)
+    many = PT.SlabSet(p, 4)
+    many.set_initial_data(u)
+    del u
+    assert one.effective_mode()[1] == 2 and all(s.effective_mode()[1] == 2 for s in many.slabs)
+    nbxy = p.nb[0] * p.nb[1]
+    for nsteps in (0, 2):
+        one.step(nsteps)
+        many.step(nsteps)
+        one.sync()
+        many.sync()
+        for r, s in enumerate(many.slabs):
+            bz0, nbz = many.parts[r]
+            assert torch.equal(s.state, one.state[:, bz0 * nbxy:(bz0 + nbz) * nbxy]), (nsteps, r)
+    assert float((one.state[I.CHI] - 1.0).abs().max()) > 0.5           # punctures: chi -> 0 near them
+    c1, cm = one.constraints(), many.constraints()
+    assert np.array_equal(cm[1::2], c1[1::2]) and np.all(np.abs(cm - c1) <= 1e-12 * np.abs(c1))
+    one.close()
+    many.close()
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
