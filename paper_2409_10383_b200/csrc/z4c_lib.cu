@@ -168,17 +168,17 @@ int launch_stage_update(z4c_ctx* c, int stage, bool push) {
 // state and its ghost images written to ybuf[1-in].
 template <class Cfg>
 cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, const RegMaps& rm, int stage,
-                                 const StageArgs& sa) {
+                                 const StageArgs& sa, int out_buf) {
   switch (stage) {
-    case 1: return launch_rhs_tiled_t<Cfg, 1>(map, rm, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
-    case 2: return launch_rhs_tiled_t<Cfg, 2>(map, rm, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa);
-    case 3: return launch_rhs_tiled_t<Cfg, 3>(map, rm, c->g, c->P, c->fd, c->sp, -0.5, c->dt, c->stream, sa);
-    default: return launch_rhs_tiled_t<Cfg, 4>(map, rm, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa);
+    case 1: return launch_rhs_tiled_t<Cfg, 1>(map, rm, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa, out_buf);
+    case 2: return launch_rhs_tiled_t<Cfg, 2>(map, rm, c->g, c->P, c->fd, c->sp, 0.0, c->dt, c->stream, sa, out_buf);
+    case 3: return launch_rhs_tiled_t<Cfg, 3>(map, rm, c->g, c->P, c->fd, c->sp, -0.5, c->dt, c->stream, sa, out_buf);
+    default: return launch_rhs_tiled_t<Cfg, 4>(map, rm, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa, out_buf);
   }
 }
 int launch_fused_stage(z4c_ctx* c, int stage, int in) {
   StageArgs sa{c->ybuf[in], c->Q, make_slab(c, 1 - in), c->prm.chi_floor, c->flag};
-  cudaError_t e = launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa);
+  cudaError_t e = launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa, 1 - in);
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
   return check_launch(c, "k_rhs_tiled<stage>");
 }
@@ -421,6 +421,8 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
                  make_state_tensor_map<RhsTile>(c->g, c->ybuf[1], &c->ymap[1]) &&
                  make_register_tensor_map<RhsTile>(c->g, c->P, &c->rmap.p) &&
                  make_register_tensor_map<RhsTile>(c->g, c->Q, &c->rmap.q) &&
+                 make_state_tensor_map<RhsTile>(c->g, c->ybuf[0], &c->rmap.o[0], true) &&
+                 make_state_tensor_map<RhsTile>(c->g, c->ybuf[1], &c->rmap.o[1], true) &&
                  configure_rhs_tiled<RhsTile>() == cudaSuccess ? 1 : 0;
   cudaError_t e = cudaMemsetAsync(d_work, 0, z4c_workspace_bytes(p), c->stream);
   if (e != cudaSuccess) {

@@ -55,6 +55,19 @@ __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* m
       : "memory");
 }
 
+// shared -> global box store (the reverse of tma_load_5d); elements outside the tensor's extents are not written
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* map, const void* smem_src, int c0, int c1, int c2,
+                                             int c3, int c4) {
+  asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
+               ::"l"(map), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// the issuing thread: shared memory of all its committed stores has been read (it may be reused / released)
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// generic-proxy writes to shared memory made visible to the async proxy (TMA) that will read them
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // ---- tile geometry ---------------------------------------------------------------------------------
 // PQ_TMA_: true = the CTA's P/Q register tiles are TMA-prefetched into shared memory at kernel start;
 // false = they are read in the epilogue as one batch of independent global loads (lines requested into L2 by a
@@ -336,7 +349,8 @@ struct StageArgs {
 template <class Cfg, int STAGE>
 __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     k_rhs_tiled(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap pmap,
-                const __grid_constant__ CUtensorMap qmap, Pack g, double* __restrict__ Preg, FdConst fd, SrcParams sp,
+                const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUtensorMap omap, Pack g,
+                double* __restrict__ Preg, FdConst fd, SrcParams sp,
                 double c, double dt, int tiles_y, int b0, StageArgs sa) {
   static_assert(Cfg::NSTAGE >= 3, "the three shift components are staged together");
   extern __shared__ __align__(128) unsigned char tiles[];   // NSTAGE halo tiles, then the mbarriers
@@ -397,8 +411,9 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
       const int nbl = a == 0 ? g.nb[0] : (a == 1 ? g.nb[1] : sa.out.nbz_global), bco = a == 0 ? bx : (a == 1 ? by : bz);
       int* L = lists + a * 3 * Cfg::MAXLIST;
       const int l = c0 + lane;
+      const int na = min(T, g.n - c0);                              // source cells of the tile on this axis
       int tb[NG + 1], tl[NG + 1];
-      const int nt = (lane < T && l < g.n) ? push_targets(l, bco, g.n, nbl, g.bc, tb, tl) : 0;
+      const int nt = lane < na ? push_targets(l, bco, g.n, nbl, g.bc, tb, tl) : 0;
       if (a == 2) {   // z targets: (table entry of the pack that holds the block) << 24 | block z inside that pack
 #pragma unroll
         for (int q = 0; q < NG + 1; ++q)
@@ -407,19 +422,23 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
             tb[q] = (e << 24) | (tb[q] - slab_bz0(sa.out, e));
           }
       }
-      int incl = nt;
+      // list order: the cells' own positions first (entry = source cell), then the ghost images; so the tile's own
+      // box is the corner [0, na)^3 of the product of the three lists and the images are the rest
+      const int ni = nt > 0 ? nt - 1 : 0;
+      int incl = ni;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         const int up = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += up;
       }
-      const int pos = incl - nt;
+      const int pos = na + incl - ni;
 #pragma unroll
       for (int q = 0; q < NG + 1; ++q)
         if (q < nt) {
-          L[pos + q] = lane; L[Cfg::MAXLIST + pos + q] = tb[q]; L[2 * Cfg::MAXLIST + pos + q] = tl[q];
+          const int at = q == 0 ? lane : pos + q - 1;
+          L[at] = lane; L[Cfg::MAXLIST + at] = tb[q]; L[2 * Cfg::MAXLIST + at] = tl[q];
         }
-      if (lane == 31) lists[9 * Cfg::MAXLIST + a] = incl;
+      if (lane == 31) lists[9 * Cfg::MAXLIST + a] = na + incl;
     }
   }
   const int toff = (lz + NG) * Cfg::SZ + (ly + NG) * Cfg::SY + lx + NG;
@@ -514,6 +533,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     return;
   }
   if (STAGE >= 2 && Cfg::PQ_TMA) mbar_wait(pqbar, 0);
+  // (without PQ_TMA the two tiles could be staged in the idle ring; measured at 4 ghosts: 0.4 % slower than plain stores)
+  constexpr bool PQ_BOX_STORE = STAGE <= 3 && Cfg::PQ_TMA;
+  double* stP = reinterpret_cast<double*>(tiles + Cfg::S_OFF);
+  double* stQ = sQ;
   if (active) {
     double* qc = sa.Q + ci;
     // without PQ_TMA: all loads of the RK registers first, as one batch of independent requests (the stores to P/Q
@@ -526,22 +549,26 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     }
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
+      // With PQ_TMA the new register values go to shared memory -- Q over the old Q tile, P into the parking area of
+      // the advection sums (read above), each thread its own slots -- and leave as two box stores after the barrier.
+      double& Pnew = PQ_BOX_STORE ? stP[f * Cfg::THREADS + tid] : pc[f * g.is];
+      double& Qnew = PQ_BOX_STORE ? stQ[f * Cfg::THREADS + tid] : qc[f * g.is];
       if (STAGE == 1) {
         const double P = dt * out[f];
-        qc[f * g.is] = P;
+        Qnew = P;
         u[f] = u[f] + 0.5 * P;
       } else if (STAGE == 2) {
         const double P = dt * out[f];
         const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
-        pc[f * g.is] = P;
+        Pnew = P;
         u[f] = u[f] + 0.5 * (P - Q);
-        qc[f * g.is] = __dmul_rn(Q, SIXTH);
+        Qnew = __dmul_rn(Q, SIXTH);
       } else if (STAGE == 3) {
         const double P = -0.5 * (Cfg::PQ_TMA ? sP[f * Cfg::THREADS + tid] : Pold[f]) + dt * out[f];
         const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
-        pc[f * g.is] = P;
+        Pnew = P;
         u[f] = u[f] + P;
-        qc[f * g.is] = Q - P;
+        Qnew = Q - P;
       } else {
         const double P = 2.0 * (Cfg::PQ_TMA ? sP[f * Cfg::THREADS + tid] : Pold[f]) + dt * out[f];
         const double Q = Cfg::PQ_TMA ? sQ[f * Cfg::THREADS + tid] : Qold[f];
@@ -555,19 +582,63 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 #pragma unroll
     for (int f = 0; f < NF; ++f) sP[f * Cfg::THREADS + tid] = u[f];
   }
+  fence_proxy_async_smem();   // the staged tile (and the new RK registers) are read by box stores
   __syncthreads();
-  // cooperative write-out of the tile and all of its ghost images, x fastest: coalesced rows
+  // A full tile's own cells leave as ONE box store of all 22 fields; a tile cut by the block's edge (n not a multiple
+  // of the tile) goes through the loop below with the images, because its box would reach into ghost cells.
+  // The box store needs its first element on a 16-byte boundary of global memory: true for the interior of a row at
+  // 4 ghosts (offset 32 bytes), not at 3 (24 bytes: the copy engine raises an illegal-instruction fault), so the
+  // 3-ghost build writes its own cells in the loop as well.
+#ifdef Z4C_DBG_MISALIGNED_STORE
+  constexpr bool TILE_STORE = true;
+  constexpr int OX = NG + 1;
+#else
+  constexpr bool TILE_STORE = (NG * 8) % 16 == 0;
+  constexpr int OX = NG;
+#endif
+  const bool full_tile = TILE_STORE && cx + Cfg::TX <= g.n && cy + Cfg::TY <= g.n && cz + Cfg::TZ <= g.n;
+  if (tid == 0) {
+    if (full_tile) tma_store_5d(&omap, sP, cx + OX, cy + NG, cz + NG, b, 0);
+    if (PQ_BOX_STORE) {
+      // the RK registers of the tile: one box store of all 22 fields each (cells beyond the block are clipped)
+      tma_store_5d(&qmap, stQ, cx, cy, cz, b, 0);
+      if (STAGE >= 2) tma_store_5d(&pmap, stP, cx, cy, cz, b, 0);
+    }
+    tma_store_commit();
+  }
+  // cooperative write-out of the tile's ghost images, x fastest. The destinations are the product of the three
+  // per-axis lists minus the corner [0, nax) x [0, nay) x [0, naz) of own positions, enumerated as three slabs:
+  //   A: qz >= naz (all qy, qx);  B: qz < naz, qy >= nay (all qx);  C: qz < naz, qy < nay, qx >= nax
   const int* Lx = lists;
   const int* Ly = lists + 3 * Cfg::MAXLIST;
   const int* Lz = lists + 6 * Cfg::MAXLIST;
   const int ncx = lists[9 * Cfg::MAXLIST], ncy = lists[9 * Cfg::MAXLIST + 1], ncz = lists[9 * Cfg::MAXLIST + 2];
-  const int total = ncx * ncy * ncz;
-  // q -> (qx, qy, qz) with reciprocal multiplies: exact for these small ranges (q < 2^11, divisors <= 22: the
-  // quotient's fractional part stays >= 0.5/22 away from an integer, float error is ~1e-4 of that)
-  const float rcx = 1.0f / (float)ncx, rcy = 1.0f / (float)ncy;
+  const int nax = full_tile ? Cfg::TX : 0, nay = full_tile ? Cfg::TY : 0, naz = full_tile ? Cfg::TZ : 0;
+  const int wx = ncx - nax, wy = ncy - nay;
+  const int nA = (ncz - naz) * ncy * ncx, nB = naz * wy * ncx, total = nA + nB + naz * nay * wx;
+  // quotients by reciprocal multiplies: exact for these small ranges (q < 2^11, divisors <= 22: the quotient's
+  // fractional part stays >= 0.5/22 away from an integer, float error is ~1e-4 of that); unused when a width is 0
+  const float rcx = 1.0f / (float)ncx, rcy = 1.0f / (float)ncy, rwx = 1.0f / (float)wx, rwy = 1.0f / (float)wy,
+              ray = 1.0f / (float)Cfg::TY;
   for (int q = tid; q < total; q += Cfg::THREADS) {
-    const int r = (int)(((float)q + 0.5f) * rcx), qx = q - r * ncx;
-    const int qz = (int)(((float)r + 0.5f) * rcy), qy = r - qz * ncy;
+    int qx, qy, qz;
+    if (q < nA) {
+      const int r = (int)(((float)q + 0.5f) * rcx);
+      qx = q - r * ncx;
+      const int z = (int)(((float)r + 0.5f) * rcy);
+      qy = r - z * ncy;
+      qz = naz + z;
+    } else if (q < nA + nB) {
+      const int q2 = q - nA, r = (int)(((float)q2 + 0.5f) * rcx);
+      qx = q2 - r * ncx;
+      qz = (int)(((float)r + 0.5f) * rwy);
+      qy = nay + r - qz * wy;
+    } else {
+      const int q2 = q - nA - nB, r = (int)(((float)q2 + 0.5f) * rwx);
+      qx = nax + q2 - r * wx;
+      qz = (int)(((float)r + 0.5f) * ray);
+      qy = r - qz * Cfg::TY;
+    }
     const int src = (Lz[qz] * Cfg::TY + Ly[qy]) * Cfg::TX + Lx[qx];
     const int zb = Lz[Cfg::MAXLIST + qz], e = zb >> 24;            // which pack, which block z inside it
     const long long tb = ((long long)(zb & 0xffffff) * g.nb[1] + Ly[Cfg::MAXLIST + qy]) * g.nb[0] + Lx[Cfg::MAXLIST + qx];
@@ -577,6 +648,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 #pragma unroll
     for (int f = 0; f < NF; ++f) d[f * efs] = sP[f * Cfg::THREADS + src];
   }
+  if (tid == 0) tma_store_wait_read();   // shared memory stays put until the box stores have read it
 }
 
 // ---- host side -------------------------------------------------------------------------------------
@@ -601,7 +673,7 @@ inline bool rhs_tiled_supported(const Pack& g) { return g.n % 2 == 0; }   // TMA
 // Encode the 5-D tensor map (i, j, k, block, field) of the state pack with a halo-tile box. Returns false if
 // the driver entry point is unavailable or rejects the geometry (the caller then keeps the plain variant).
 template <class Cfg>
-inline bool make_state_tensor_map(const Pack& g, const double* y, CUtensorMap* out) {
+inline bool make_state_tensor_map(const Pack& g, const double* y, CUtensorMap* out, bool tile_box = false) {
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -613,7 +685,9 @@ inline bool make_state_tensor_map(const Pack& g, const double* y, CUtensorMap* o
   const cuuint64_t m = (cuuint64_t)g.m;
   const cuuint64_t dims[5] = {m, m, m, (cuuint64_t)g.nblk, (cuuint64_t)NF};
   const cuuint64_t strides[4] = {m * 8, m * m * 8, m * m * m * 8, (cuuint64_t)g.fs * 8};
-  const cuuint32_t box[5] = {(cuuint32_t)Cfg::HX, (cuuint32_t)Cfg::HY, (cuuint32_t)Cfg::HZ, 1, 1};
+  // halo tile of one field (loads), or the bare tile of all 22 fields (the store of a tile's new interior values)
+  const cuuint32_t box[5] = {(cuuint32_t)(tile_box ? Cfg::TX : Cfg::HX), (cuuint32_t)(tile_box ? Cfg::TY : Cfg::HY),
+                             (cuuint32_t)(tile_box ? Cfg::TZ : Cfg::HZ), 1, (cuuint32_t)(tile_box ? NF : 1)};
   const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
   const CUresult r = ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)y, dims, strides, box, estr,
                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -643,7 +717,7 @@ inline bool make_register_tensor_map(const Pack& g, const double* reg, CUtensorM
   return r == CUDA_SUCCESS;
 }
 
-struct RegMaps { CUtensorMap p, q; };
+struct RegMaps { CUtensorMap p, q, o[2]; };   // RK registers P, Q; the two state buffers with a bare-tile box (stores)
 
 // Shared-memory opt-in of every stage instantiation, for the CURRENT device (function attributes are per device:
 // z4c_create calls this once per context, so a process may drive several devices).
@@ -668,14 +742,14 @@ inline cudaError_t configure_rhs_tiled() {
 template <class Cfg, int STAGE>
 inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm, const Pack& g, double* P, const FdConst& fd,
                                       const SrcParams& sp, double coef, double dt, cudaStream_t st,
-                                      const StageArgs& sa) {
+                                      const StageArgs& sa, int out_buf = 0) {
   constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
   if ((long long)ty * tz > 65535) return cudaErrorInvalidConfiguration;
   for (int b0 = 0; b0 < g.nblk; b0 += 65535) {   // gridDim.z <= 65535: packs with more blocks take several launches
     const int nb = g.nblk - b0 < 65535 ? g.nblk - b0 : 65535;
-    k_rhs_tiled<Cfg, STAGE><<<dim3(tx, ty * tz, nb), Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, g, P, fd, sp, coef, dt, ty,
-                                                                                b0, sa);
+    k_rhs_tiled<Cfg, STAGE><<<dim3(tx, ty * tz, nb), Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, rm.o[out_buf], g, P, fd, sp,
+                                                                                coef, dt, ty, b0, sa);
   }
   return cudaSuccess;
 }
