@@ -47,6 +47,10 @@ CASES = {
     "o6_noise_ragged": lambda: (replace(I.params_noise(10, (2, 1, 2)), ng=4), "noise"),
     "o6_smooth_periodic": lambda: (replace(I.params_noise(16, (2, 1, 1), dx=0.05), ng=4), "smooth"),
     "o6_smooth_outflow": lambda: (replace(I.params_noise(12, (1, 2, 2), dx=0.05), ng=4, bc=1, shift_eta=1.0), "smooth"),
+    # blocks of 18^3: 16x4x2 tiles that are full (their own cells leave as one box store at 4 ghosts, the register tiles
+    # at 3) next to tiles cut in x and in y (everything through the write-out loop, box stores clipped at the block's edge)
+    "smooth_mixed_tiles": lambda: (replace(I.params_noise(18, (2, 1, 1), dx=0.05), bc=1, shift_eta=1.0), "smooth"),
+    "o6_smooth_mixed_tiles": lambda: (replace(I.params_noise(18, (1, 2, 1), dx=0.05), ng=4), "smooth"),
 }
 
 
@@ -176,7 +180,7 @@ def test_odd_block_size_runs_the_plain_kernel(Z, oracle):
 
 
 def test_fused_push_equals_separate_ghost_fill_bitwise(Z):
-    for name in ("noise_ragged", "smooth_outflow"):
+    for name in ("noise_ragged", "smooth_outflow", "smooth_mixed_tiles", "o6_smooth_mixed_tiles"):
         p, u = case_data(name)
         a = make(Z, p, u, fused=1)
         b = make(Z, p, u, fused=0)
