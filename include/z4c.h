@@ -79,8 +79,9 @@ typedef struct {
 /* Bytes of the state buffer y: 22*N_b*m^3*8. Returns 0 if the parameters are invalid. */
 size_t z4c_state_bytes(const z4c_params* p);
 
-/* Bytes of the workspace (RK registers P and Q on interior cells, reduction scratch, error flag, and the
- * second state buffer of the one-kernel-per-stage mode: about 2*22*N_b*n^3*8 + 22*N_b*m^3*8).
+/* Bytes of the workspace (RK registers P and Q on interior cells, reduction scratch, error flag, the
+ * second state buffer of the one-kernel-per-stage mode and a list of N_b block indices: about
+ * 2*22*N_b*n^3*8 + 22*N_b*m^3*8).
  * Returns 0 if the parameters are invalid. */
 size_t z4c_workspace_bytes(const z4c_params* p);
 
@@ -159,7 +160,12 @@ int z4c_refine_indicators(z4c_ctx* ctx, double chi_min, double dchi_max, double*
  *   (and once on entry, so the levels are consistent whatever the caller loaded). The set-up of the paper's
  *   refined-corner wave test. With both contexts in mode 2 (z4c_set_fused) every stage is the fused
  *   stage kernel on each level followed by the two exchange kernels on the buffer just written (4 launches per stage);
- *   otherwise RHS, update + push per level, then the exchange (6 launches per stage). Async.
+ *   otherwise RHS, update + push per level, then the exchange (6 launches per stage). In mode 2, when the region is
+ *   made of whole coarse MeshBlocks (the paper's refinement unit), the coarse blocks under it are not
+ *   advanced at all (the restriction overwrites them) and between stages only the covered cells that are read --
+ *   the N_g layers under the region's faces -- are restricted; the last stage of the call restricts every covered
+ *   cell, so on return the coarse level is complete and equal to what the full sequence gives. The list of blocks
+ *   to advance lives in the coarse context's workspace (N_b ints, counted by z4c_workspace_bytes). Async.
  * Errors: Z4C_EINVAL (different streams, spacing not 2:1, box outside the coarse mesh, odd n, unequal dt, a
  *   partitioned pack). */
 int z4c_restrict(z4c_ctx* fine, z4c_ctx* coarse, const int32_t* origin);

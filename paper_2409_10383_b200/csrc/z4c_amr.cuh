@@ -90,12 +90,19 @@ __device__ __forceinline__ int prolong_axis(const int i, const AmrWeights& t, do
 struct AmrGeom {
   int origin[3];   // coarse global cell index of the fine region's corner
   int Mc[3];       // coarse cells covered per axis = fine cells / 2
+  int layer = -1;  // k_restrict: >= 0 = only the covered cells within `layer` cells of the region's faces (what the
+                   // coarse neighbours and the prolongation read); -1 = every covered cell
 };
 
 // Step B.1: covered coarse interior cells <- restriction of the fine active cells, and steps A.2 / B.2
 // for those cells: the thread also writes the ghost images of its coarse cell (same wrap / clamp rule as O2, the
 // target list of the stage update's push), so the coarse level needs no whole-pack ghost fill after a restriction.
 // One thread per (covered coarse cell, field).
+// cells within a.layer of the region's faces (the launcher only sets a layer with 2 * layer <= every extent)
+__host__ __device__ inline long long restrict_layer_cells(const AmrGeom& a) {
+  const long long Mx = a.Mc[0], My = a.Mc[1], Mz = a.Mc[2], L2 = 2 * a.layer;
+  return Mx * My * Mz - (Mx - L2) * (My - L2) * (Mz - L2);
+}
 constexpr int RB_X = 16, RB_Y = 4, RB_Z = 2;   // k_restrict's brick of coarse cells per CTA (128 threads)
 __global__ void __launch_bounds__(RB_X * RB_Y * RB_Z) k_restrict(Pack gf, const double* __restrict__ yf, Pack gc,
                                                   double* __restrict__ yc, AmrGeom a, AmrWeights wt) {
@@ -104,9 +111,30 @@ __global__ void __launch_bounds__(RB_X * RB_Y * RB_Z) k_restrict(Pack gf, const 
   const int bricks_x = (a.Mc[0] + RB_X - 1) / RB_X, bricks_y = (a.Mc[1] + RB_Y - 1) / RB_Y;
   const int f = blockIdx.y;
   const int bx = blockIdx.x % bricks_x, by = (blockIdx.x / bricks_x) % bricks_y, bz = blockIdx.x / (bricks_x * bricks_y);
-  const int C[3] = {bx * RB_X + (int)(threadIdx.x % RB_X), by * RB_Y + (int)((threadIdx.x / RB_X) % RB_Y),
-                    bz * RB_Z + (int)(threadIdx.x / (RB_X * RB_Y))};
-  if (C[0] >= a.Mc[0] || C[1] >= a.Mc[1] || C[2] >= a.Mc[2]) return;
+  int C[3] = {bx * RB_X + (int)(threadIdx.x % RB_X), by * RB_Y + (int)((threadIdx.x / RB_X) % RB_Y),
+              bz * RB_Z + (int)(threadIdx.x / (RB_X * RB_Y))};
+  if (a.layer >= 0) {
+    // only the `layer` cells under each face of the region, enumerated directly: z-slabs, y-slabs, x-slabs
+    const int L2 = 2 * a.layer, Mx = a.Mc[0], My = a.Mc[1], Mz = a.Mc[2];
+    const long long nZ = (long long)L2 * My * Mx, nY = (long long)(Mz - L2) * L2 * Mx;
+    long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (r >= restrict_layer_cells(a)) return;
+    if (r < nZ) {
+      const int zz = (int)(r / ((long long)My * Mx));
+      C[0] = (int)(r % Mx); C[1] = (int)((r / Mx) % My); C[2] = zz < a.layer ? zz : Mz - L2 + zz;
+    } else if (r < nZ + nY) {
+      r -= nZ;
+      const int q = (int)((r / Mx) % L2);
+      C[0] = (int)(r % Mx); C[1] = q < a.layer ? q : My - L2 + q; C[2] = a.layer + (int)(r / ((long long)L2 * Mx));
+    } else {
+      r -= nZ + nY;
+      const int q = (int)(r % L2);
+      C[0] = q < a.layer ? q : Mx - L2 + q; C[1] = a.layer + (int)((r / L2) % (My - L2));
+      C[2] = a.layer + (int)(r / ((long long)L2 * (My - L2)));
+    }
+  } else if (C[0] >= a.Mc[0] || C[1] >= a.Mc[1] || C[2] >= a.Mc[2]) {
+    return;
+  }
   double w[3][AMR_N];
   int s[3], fb[3], ref[3];
   const int half = gf.n / 2;

@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/z4c.h"
 #include "z4c_amr.cuh"
@@ -46,6 +47,10 @@ struct z4c_ctx {
   int bz0, nbz_global;
   double* nbr_y[2][2];   // [lower, upper][state buffer 0, 1] of the neighbouring slabs (peer memory), or null
   int nbr_bz0[2], nbr_nbz[2];
+  // NEXT-3: list of the blocks a two-level step advances on this (coarse) pack -- all but those a fine level covers
+  int* blist;            // device, workspace: N_b ints
+  int nactive;           // entries of blist in use; -1 = no list (every block runs)
+  int blist_key[6];      // origin and extent of the fine region the list was built for
   std::string err;
 };
 
@@ -176,8 +181,13 @@ cudaError_t launch_fused_stage_t(z4c_ctx* c, const CUtensorMap& map, const RegMa
     default: return launch_rhs_tiled_t<Cfg, 4>(map, rm, c->g, c->P, c->fd, c->sp, 2.0, c->dt, c->stream, sa, out_buf);
   }
 }
-int launch_fused_stage(z4c_ctx* c, int stage, int in) {
+int launch_fused_stage(z4c_ctx* c, int stage, int in, bool listed_blocks_only = false) {
   StageArgs sa{c->ybuf[in], c->Q, make_slab(c, 1 - in), c->prm.chi_floor, c->flag};
+  if (listed_blocks_only && c->nactive >= 0) {
+    if (c->nactive == 0) return Z4C_OK;   // a fine level covers the whole pack
+    sa.blist = c->blist;
+    sa.nrun = c->nactive;
+  }
   cudaError_t e = launch_fused_stage_t<RhsTile>(c, c->ymap[in], c->rmap, stage, sa, 1 - in);
   if (e != cudaSuccess) return check_cuda(c, e, "k_rhs_tiled launch");
   return check_launch(c, "k_rhs_tiled<stage>");
@@ -358,7 +368,7 @@ size_t z4c_workspace_bytes(const z4c_params* p) {
   const Pack g = make_pack(*p);
   const size_t reg = align_up((size_t)NF * (size_t)g.is * sizeof(double));
   return 2 * reg + align_up((size_t)K4_MAX_PARTS * 8 * sizeof(double)) + align_up(8 * sizeof(double)) + ALIGN +
-         align_up((size_t)NF * (size_t)g.fs * sizeof(double));
+         align_up((size_t)NF * (size_t)g.fs * sizeof(double)) + align_up((size_t)g.nblk * sizeof(int));
 }
 
 int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stream, z4c_ctx** out) {
@@ -396,6 +406,8 @@ int z4c_create(const z4c_params* p, void* d_state, void* d_work, void* cuda_stre
   c->flag = (int*)((char*)c->result + align_up(8 * sizeof(double)));
   c->ybuf[0] = c->y;
   c->ybuf[1] = (double*)((char*)c->flag + ALIGN);
+  c->blist = (int*)((char*)c->ybuf[1] + align_up((size_t)NF * (size_t)c->g.fs * sizeof(double)));
+  c->nactive = -1;
   c->stream = (cudaStream_t)cuda_stream;
   c->steps = 0;
   c->launches = 0;
@@ -618,8 +630,9 @@ int check_levels(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, AmrGeom*
   return Z4C_OK;
 }
 int launch_restrict(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
-  const long long bricks = (long long)((a.Mc[0] + RB_X - 1) / RB_X) * ((a.Mc[1] + RB_Y - 1) / RB_Y) *
-                           ((a.Mc[2] + RB_Z - 1) / RB_Z);
+  const long long bricks = a.layer >= 0 ? (restrict_layer_cells(a) + RB_X * RB_Y * RB_Z - 1) / (RB_X * RB_Y * RB_Z)
+                                        : (long long)((a.Mc[0] + RB_X - 1) / RB_X) * ((a.Mc[1] + RB_Y - 1) / RB_Y) *
+                                              ((a.Mc[2] + RB_Z - 1) / RB_Z);
   if (bricks > 0x7fffffffLL) return fail(fine, Z4C_EINVAL, "fine region too large for one k_restrict launch");
   k_restrict<<<dim3((unsigned)bricks, NF), RB_X * RB_Y * RB_Z, 0, fine->stream>>>(
       fine->g, fine->ybuf[buf], coarse->g, coarse->ybuf[buf], a, make_amr_weights(fine->g.n));
@@ -632,6 +645,28 @@ int launch_prolong(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0
                                                                                fine->ybuf[buf], a,
                                                                                make_amr_weights(g.n));
   return check_launch(fine, "k_prolong");
+}
+// The coarse blocks that are not completely covered by the fine region, in pack order, into the workspace's list.
+int list_uncovered_blocks(z4c_ctx* coarse, const AmrGeom& a) {
+  const int key[6] = {a.origin[0], a.origin[1], a.origin[2], a.Mc[0], a.Mc[1], a.Mc[2]};
+  if (coarse->nactive >= 0 && std::memcmp(key, coarse->blist_key, sizeof(key)) == 0) return Z4C_OK;
+  const Pack& g = coarse->g;
+  std::vector<int> list;
+  list.reserve(g.nblk);
+  for (int b = 0; b < g.nblk; ++b) {
+    const int bx = b % g.nb[0], by = (b / g.nb[0]) % g.nb[1], bz = b / (g.nb[0] * g.nb[1]);
+    const int lo[3] = {bx * g.n, by * g.n, bz * g.n};
+    bool covered = true;
+    for (int d = 0; d < 3; ++d) covered = covered && lo[d] >= a.origin[d] && lo[d] + g.n <= a.origin[d] + a.Mc[d];
+    if (!covered) list.push_back(b);
+  }
+  // pageable source: the copy is staged before the call returns, so the vector may go
+  int rc = check_cuda(coarse, cudaMemcpyAsync(coarse->blist, list.data(), list.size() * sizeof(int), cudaMemcpyHostToDevice,
+                                              coarse->stream), "block list copy");
+  if (rc) return rc;
+  coarse->nactive = (int)list.size();
+  std::memcpy(coarse->blist_key, key, sizeof(key));
+  return Z4C_OK;
 }
 // steps B.1, A.2/B.2 (k_restrict writes the ghost images of the covered coarse nodes itself), B.5; on state buffer `buf`
 int sync_levels(z4c_ctx* coarse, z4c_ctx* fine, const AmrGeom& a, int buf = 0) {
@@ -667,13 +702,26 @@ int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, in
   // Both levels in mode 2: one stage kernel per level and stage (state ping-pong ybuf[in] -> ybuf[1 - in], ghost images
   // written by the kernel), then the level exchange on the buffer just written. Otherwise K2 + K3-with-push in place.
   const bool fused = fully_fused(coarse) && fully_fused(fine);
+  // A region made of whole coarse blocks (the paper's refinement unit): whatever the coarse stage kernel
+  // computes on those blocks is overwritten by the restriction, so they are not advanced at all, and between stages
+  // only the covered cells that anyone reads are restricted: the N_g layers under the region's faces (ghost images
+  // of the coarse neighbours, step A.2 / B.2; the prolongation stencils reach 2 nodes in). The last stage of the call
+  // restricts every covered cell, so the caller finds the coarse level complete.
+  bool whole_blocks = fused && rc == Z4C_OK;
+  for (int d = 0; d < 3; ++d) whole_blocks = whole_blocks && a.origin[d] % coarse->g.n == 0 && a.Mc[d] % coarse->g.n == 0;
+  if (whole_blocks) rc = list_uncovered_blocks(coarse, a);
+  AmrGeom faces = a;
+  faces.layer = NG;
+  for (int d = 0; d < 3; ++d) if (2 * NG > a.Mc[d]) faces.layer = -1;   // a region thinner than two layers: all of it
   z4c_ctx* lv[2] = {coarse, fine};
   for (int st = 0; st < nsteps && rc == Z4C_OK; ++st)
     for (int s = 1; s <= 4 && rc == Z4C_OK; ++s) {
       const int in = (s - 1) & 1;
       if (fused) {
-        for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_fused_stage(lv[q], s, in);
-        if (rc == Z4C_OK) rc = sync_levels(coarse, fine, a, 1 - in);
+        rc = launch_fused_stage(coarse, s, in, whole_blocks);
+        if (rc == Z4C_OK) rc = launch_fused_stage(fine, s, in);
+        const bool last = st == nsteps - 1 && s == 4;
+        if (rc == Z4C_OK) rc = sync_levels(coarse, fine, whole_blocks && !last ? faces : a, 1 - in);
       } else {
         for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_rhs(lv[q], coef[s - 1], lv[q]->dt);
         for (int q = 0; q < 2 && rc == Z4C_OK; ++q) rc = launch_stage_update(lv[q], s, true);

@@ -341,6 +341,8 @@ struct StageArgs {
                         // other buffers of the z-neighbours' packs (peer memory)
   double chi_floor;
   int* flag;
+  const int* blist = nullptr;   // blocks to run (device, nrun entries), or null: all blocks of the pack in order
+  int nrun = 0;                 // (NEXT-3: the coarse blocks a fine level covers completely are not advanced)
 };
 
 // STAGE 0: P <- c*P + dt*(F(y) + Q_KO(y)) only (z4c_eval_rhs and the unfused path).
@@ -364,7 +366,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
   const int lx = tid % Cfg::TX, ly = (tid / Cfg::TX) % Cfg::TY, lz = tid / (Cfg::TX * Cfg::TY);
   // grid = (tiles_x, tiles_y * tiles_z, blocks of this launch): one integer division per CTA instead of three
   const int tx = blockIdx.x, tz = blockIdx.y / tiles_y, ty = blockIdx.y - tz * tiles_y;
-  const int b = b0 + blockIdx.z;
+  const int b = sa.blist ? sa.blist[b0 + blockIdx.z] : b0 + blockIdx.z;
   // padded coordinates of the halo tile's origin = interior coordinates of the tile's first cell
   const int cx = tx * Cfg::TX, cy = ty * Cfg::TY, cz = tz * Cfg::TZ;
   const int i = cx + lx, j = cy + ly, k = cz + lz;
@@ -746,8 +748,9 @@ inline cudaError_t launch_rhs_tiled_t(const CUtensorMap& map, const RegMaps& rm,
   constexpr int smem = STAGE == 0 ? Cfg::SMEM_BYTES_RHS : Cfg::SMEM_BYTES;
   const int tx = (g.n + Cfg::TX - 1) / Cfg::TX, ty = (g.n + Cfg::TY - 1) / Cfg::TY, tz = (g.n + Cfg::TZ - 1) / Cfg::TZ;
   if ((long long)ty * tz > 65535) return cudaErrorInvalidConfiguration;
-  for (int b0 = 0; b0 < g.nblk; b0 += 65535) {   // gridDim.z <= 65535: packs with more blocks take several launches
-    const int nb = g.nblk - b0 < 65535 ? g.nblk - b0 : 65535;
+  const int nrun = sa.blist ? sa.nrun : g.nblk;
+  for (int b0 = 0; b0 < nrun; b0 += 65535) {     // gridDim.z <= 65535: packs with more blocks take several launches
+    const int nb = nrun - b0 < 65535 ? nrun - b0 : 65535;
     k_rhs_tiled<Cfg, STAGE><<<dim3(tx, ty * tz, nb), Cfg::THREADS, smem, st>>>(map, rm.p, rm.q, rm.o[out_buf], g, P, fd, sp,
                                                                                 coef, dt, ty, b0, sa);
   }
