@@ -106,3 +106,23 @@ def test_workload_params_and_slab_data_agree_with_the_configs():
     for r in range(3):
         ps = PT.slab_params(p, r, 3)
         assert np.array_equal(bench.workload_data("bbh_256", ps), PT.slab_interior(whole, p, r, 3))
+
+
+def test_two_level_workload_geometry():
+    """bench.py --workload two_level_wave_256: the fine pack is the 2:1 refinement of a box of whole coarse blocks
+    inside the coarse mesh, both levels share one dt, and the small (oracle-sized) variant has the same shape."""
+    sys.path.insert(0, ROOT)
+    import bench
+    for small in (False, True):
+        pc, pf, origin = bench.two_level_workload(small=small)
+        assert abs(2.0 * pf.dx - pc.dx) < 1e-15 and abs(pc.dt - pf.dt) < 1e-18
+        assert pc.bc == 0 and pf.bc == 1 and pc.ng == pf.ng
+        for d in range(3):
+            Mc = pf.N[d] // 2
+            assert pf.N[d] % 2 == 0
+            if not small:                                   # the timed mesh refines whole coarse blocks
+                assert origin[d] % pc.n == 0 and Mc % pc.n == 0
+            assert 0 <= origin[d] and origin[d] + Mc <= pc.N[d]
+            assert abs(pf.xmin[d] - (pc.xmin[d] + origin[d] * pc.dx)) < 1e-14                # same physical corner
+    pc, pf, origin = bench.two_level_workload()
+    assert pc.nblocks == 512 and pf.nblocks == 512 and pc.n == 32 and pf.n == 32
