@@ -198,6 +198,12 @@ int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, in
  * z4c_constraints_raw: like z4c_constraints but the four sums of squares are NOT divided and rooted:
  *   out = {sum H^2, max|H|, sum |M|^2, max|M|, sum Theta^2, max|Theta|, sum |Z|^2, max|Z|} over this slab, so that the
  *   mesh-wide norms are one 8-double all-reduce away (SUM on even, MAX on odd entries). Synchronises the stream. */
+/* z4c_enable_peer: lets kernels launched on the CURRENT device store into memory that lives on `peer_device`
+ *   (cudaDeviceEnablePeerAccess; already-enabled access is not an error; the current device itself is accepted and
+ *   needs nothing). Call it once per neighbour on another GPU before the first z4c_stage: opening a neighbour's
+ *   buffers through CUDA IPC maps them, it does not by itself let this GPU's kernels reach them.
+ *   Errors: Z4C_ECUDA (no such device, or the two GPUs cannot reach each other). */
+int z4c_enable_peer(int32_t peer_device);
 int z4c_set_partition(z4c_ctx* ctx, int32_t nbz_global, int32_t bz0);
 int z4c_set_neighbor(z4c_ctx* ctx, int32_t side, void* d_state, void* d_state2, int32_t bz0, int32_t nbz);
 void* z4c_state2(const z4c_ctx* ctx);

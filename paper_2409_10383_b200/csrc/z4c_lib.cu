@@ -733,6 +733,21 @@ int z4c_two_level_step(z4c_ctx* coarse, z4c_ctx* fine, const int32_t* origin, in
 }
 
 // ---- NEXT-2: partitioned mesh (ghost exchange at every stage) -----------
+int z4c_enable_peer(int32_t peer_device) {
+  int dev = -1, count = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceCount(&count) != cudaSuccess) return Z4C_ECUDA;
+  if (peer_device < 0 || peer_device >= count) return Z4C_ECUDA;
+  if (peer_device == dev) return Z4C_OK;
+  int can = 0;
+  if (cudaDeviceCanAccessPeer(&can, dev, peer_device) != cudaSuccess || !can) return Z4C_ECUDA;
+  const cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
+  if (e == cudaErrorPeerAccessAlreadyEnabled) {
+    cudaGetLastError();   // not an error: clear it
+    return Z4C_OK;
+  }
+  return e == cudaSuccess ? Z4C_OK : Z4C_ECUDA;
+}
+
 int z4c_set_partition(z4c_ctx* c, int32_t nbz_global, int32_t bz0) {
   if (!c) return Z4C_EINVAL;
   if (bz0 < 0 || nbz_global < 1 || bz0 + c->g.nb[2] > nbz_global || nbz_global > (1 << 24)) return Z4C_EINVAL;

@@ -154,6 +154,7 @@ class DistributedSlab:
             (f_state, a_state), (f_work, a_work), off2 = everyone[nb]
             st, wk = f_state(*a_state), f_work(*a_work)        # tensors aliasing the neighbour's memory
             self._peer_tensors += [st, wk]
+            self.sim.enable_peer(st.device.index)              # another GPU: let this GPU's kernels store into it
             self.sim.set_neighbor(side, st.data_ptr(), wk.data_ptr() + off2, *self.parts[nb])
         self.barrier()
 

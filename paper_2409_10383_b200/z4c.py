@@ -24,7 +24,7 @@ SYMBOLS = ["z4c_state_bytes", "z4c_workspace_bytes", "z4c_create", "z4c_set_init
            "z4c_launch_count", "z4c_set_variant", "z4c_use_graph", "z4c_set_fused", "z4c_step_timed",
            "z4c_probe_fp64", "z4c_effective_mode", "z4c_time",
            "z4c_restrict", "z4c_prolongate", "z4c_two_level_step",
-           "z4c_set_partition", "z4c_set_neighbor", "z4c_state2", "z4c_stage", "z4c_stage_rhs", "z4c_stage_update",
+           "z4c_enable_peer", "z4c_set_partition", "z4c_set_neighbor", "z4c_state2", "z4c_stage", "z4c_stage_rhs", "z4c_stage_update",
            "z4c_constraints_raw",
            "z4c_last_error", "z4c_destroy"]
 
@@ -103,6 +103,7 @@ def load_library(path: Optional[str] = None, ng: int = 3):
     L.z4c_stage_rhs.argtypes = [vp, C.c_int]
     L.z4c_stage_update.argtypes = [vp, C.c_int]
     L.z4c_constraints_raw.argtypes = [vp, C.POINTER(C.c_double)]
+    L.z4c_enable_peer.argtypes = [C.c_int32]
     L.z4c_time.argtypes = [vp]
     L.z4c_time.restype = C.c_double
     L.z4c_last_error.argtypes = [vp]
@@ -330,6 +331,13 @@ class Z4c:
             self._check(self.lib.z4c_two_level_step(coarse.h, self.h, o, int(nsteps)))
 
     # -- NEXT-2: one slab of a partitioned mesh ------------------------------------------------------------
+    def enable_peer(self, peer_device: int):
+        """z4c_enable_peer with this context's device current: its kernels may then store into `peer_device`'s memory."""
+        with self.torch.cuda.device(self.device):
+            rc = self.lib.z4c_enable_peer(int(peer_device))
+        if rc != 0:
+            raise Z4cError(rc, f"z4c_enable_peer({peer_device}) failed: no such device, or no peer path from {self.device}")
+
     def set_partition(self, nbz_global: int, bz0: int):
         self._check(self.lib.z4c_set_partition(self.h, int(nbz_global), int(bz0)))
 

@@ -105,6 +105,24 @@ def test_config3_in_four_slabs_at_full_size_bitwise(Z):
     many.close()
 
 
+def test_enable_peer_on_the_own_device_and_on_a_missing_one(Z):
+    import torch
+    p = I.params_noise(16, (1, 1, 1), dx=0.05)
+    sim = Z.Z4c(p)
+    sim.set_initial_data(I.noise_data(p, 3))
+    sim.enable_peer(torch.cuda.current_device())        # the own device needs nothing
+    sim.enable_peer(torch.cuda.current_device())        # twice is not an error either
+    with pytest.raises(Z.Z4cError):
+        sim.enable_peer(torch.cuda.device_count() + 7)
+    for other in range(torch.cuda.device_count()):      # on a multi-GPU node: every reachable peer, twice
+        if other != torch.cuda.current_device() and torch.cuda.can_device_access_peer(torch.cuda.current_device(), other):
+            sim.enable_peer(other)
+            sim.enable_peer(other)
+    sim.step(1)                                          # the context still works (no sticky error left behind)
+    sim.sync()
+    sim.close()
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
