@@ -82,9 +82,10 @@ struct TileCfg {
   static constexpr int TILE_ELEMS = HX * HY * HZ;
   static constexpr int TILE_BYTES = TILE_ELEMS * 8;
   static constexpr int STAGE_BYTES = (TILE_BYTES + 127) / 128 * 128;
-  // With the RK-register tiles in shared memory a 4th ring slot lives in the Q tile's area, which is idle during the
-  // field stream (both register tiles are then asked for after the stream).
-  static constexpr int PHYS = (PQ_TMA_ && NSTAGE_ == 4) ? 3 : NSTAGE_;
+  // With the RK-register tiles in shared memory a 4th ring slot lives at the end of the Q tile's area, which is idle
+  // during the field stream (both register tiles are then asked for after the stream), and a 5th one behind the plane
+  // set in the P tile's area, reaching a little into the front of the Q area.
+  static constexpr int PHYS = (PQ_TMA_ && (NSTAGE_ == 4 || NSTAGE_ == 5)) ? 3 : NSTAGE_;
   static constexpr int BAR_OFF = PHYS * STAGE_BYTES;              // NSTAGE + 1 mbarriers
   static constexpr int REG_BYTES = NF * THREADS * 8;              // one RK-register tile [22][TZ][TY][TX]
   static constexpr int P_OFF = BAR_OFF + 128;                     // P tile, later the staged new state
@@ -106,8 +107,13 @@ struct TileCfg {
   static_assert(!PQ_TMA || MIX_BYTES <= REG_BYTES, "the planes fit the P tile area (the Q tile arrives during the stream)");
   static constexpr int LIST_OFF = E_OFF + (EARLY_PARK ? NPARK * THREADS * 8 : 0) + (PQ_TMA ? 0 : MIX_BYTES);   // push lists
   static constexpr int MAXLIST = 32;
-  __host__ __device__ static constexpr int slot_off(int s) { return s < PHYS ? s * STAGE_BYTES : Q_OFF; }
-  static_assert(PHYS == NSTAGE_ || STAGE_BYTES <= REG_BYTES, "the 4th slot fits the Q tile area");
+  __host__ __device__ static constexpr int slot_off(int s) {
+    return s < PHYS ? s * STAGE_BYTES : (s == PHYS ? Q_OFF + REG_BYTES - STAGE_BYTES : P_OFF + MIX_BYTES);
+  }
+  static_assert(PHYS == NSTAGE_ || (STAGE_BYTES <= REG_BYTES && (REG_BYTES - STAGE_BYTES) % 128 == 0),
+                "the 4th slot fits the end of the Q tile area");
+  static_assert(NSTAGE_ - PHYS < 2 || P_OFF + MIX_BYTES + STAGE_BYTES <= Q_OFF + REG_BYTES - STAGE_BYTES,
+                "the 5th slot ends before the 4th begins");
   static constexpr int SMEM_BYTES_RHS = LIST_OFF;                 // STAGE 0 (no lists)
   static constexpr int SMEM_BYTES = LIST_OFF + 9 * MAXLIST * 4 + 16;
   static_assert(TX + 2 * NG <= MAXLIST && TY + 2 * NG <= MAXLIST && TZ + 2 * NG <= MAXLIST, "push list size");
@@ -662,9 +668,10 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
 //   8-wide tiles (8x4x4, 8x8x2: 20 % fewer halo bytes) are 20 % slower: 64-byte rows halve the coalescing of the
 //   register / state rows and put two tile rows of a warp on the same shared-memory banks.
 #if Z4C_NG == 3
-// 4-deep ring: three slots of their own, the 4th in the Q tile's area (+1.1 % on configs[3], +1.6 % on configs[1] over
-// the 3-deep ring with the Q tile asked for during the stream)
-using RhsTile = TileCfg<16, 4, 2, 4, 2>;
+// 5-deep ring: three slots of their own, the 4th at the end of the Q tile's area (+1.1 % on configs[3], +1.6 % on
+// configs[1] over the 3-deep ring with the Q tile asked for during the stream), the 5th behind the plane set in the P
+// tile's area (another +0.4 % / +0.9 %)
+using RhsTile = TileCfg<16, 4, 2, 5, 2>;
 #else
 // 4 ghosts: the halo tile grows to 24 x 12 x 10 (23 KB); to keep 2 CTAs per SM the P/Q tiles are read by batched
 // global loads instead of TMA (93 KB of shared memory per CTA)
