@@ -395,26 +395,27 @@ __global__ void __launch_bounds__(Cfg::THREADS, Cfg::MINB)
     for (int s = 0; s < Cfg::NSTAGE; ++s) mbar_init(&full[s], 1);
     mbar_init(pqbar, (STAGE >= 3 && Cfg::PHYS == Cfg::NSTAGE) ? 2 : 1);   // one arrival per RK-register tile asked for (Q early, P late)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  if (tid == 0) {
+    // the first tiles are asked for by the thread that set the barriers up, before the CTA barrier (which only keeps
+    // the other threads from polling a barrier that is not there yet)
 #pragma unroll
     for (int s = 0; s < Cfg::NSTAGE; ++s) {
       mbar_expect_tx(&full[s], Cfg::TILE_BYTES);
       tma_load_5d(tiles + Cfg::slot_off(s), &map, &full[s], cx, cy, cz, b, stream_field(s));
     }
   }
+  __syncthreads();
   // push lists (O2): per axis, every (source cell of this tile -> destination block, padded index) pair, the
-  // cell's own position included; the destinations of the tile are the product of the three lists. Built by the
-  // LAST warp, one lane per source cell with a warp prefix sum for the list positions: a few dozen instructions,
-  // so that no warp arrives late at the first barrier (a serial build by thread 0 cost ~1 us per CTA).
-  if (STAGE >= 1 && tid >= Cfg::THREADS - 32) {
+  // cell's own position included; the destinations of the tile are the product of the three lists. Built by warps
+  // 1..3, one axis each, one lane per source cell with a warp prefix sum for the list positions: a few dozen
+  // instructions, so that no warp arrives late at the first barrier (a serial build by thread 0 cost ~1 us per CTA).
+  static_assert(Cfg::THREADS == 128, "warps 1..3 build the lists of the axes x, y, z");
+  if (STAGE >= 1 && tid >= 32) {
     const int lane = tid & 31;
     int bx, by, bz;
     block_coords(g, b, bx, by, bz);
     bz += sa.out.bz0[0];                                          // z in the lattice of the whole mesh (NEXT-2)
-#pragma unroll 1   // one copy of the body for the three axes: off the critical path, and code size is not free here
-    for (int a = 0; a < 3; ++a) {
+    {   // one copy of the body, run by three warps side by side (warp 0 holds the thread that issues the tile copies)
+      const int a = (tid >> 5) - 1;
       const int c0 = a == 0 ? cx : (a == 1 ? cy : cz), T = a == 0 ? Cfg::TX : (a == 1 ? Cfg::TY : Cfg::TZ);
       const int nbl = a == 0 ? g.nb[0] : (a == 1 ? g.nb[1] : sa.out.nbz_global), bco = a == 0 ? bx : (a == 1 ? by : bz);
       int* L = lists + a * 3 * Cfg::MAXLIST;
