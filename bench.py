@@ -246,8 +246,14 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    r = time_oracle(args.workload, args.steps, args.warmup, budget_s=60.0)
-    label = WORKLOAD_LABELS.get(args.workload, args.workload)
+    if args.workload == "two_level_wave_256":
+        c = time_oracle_two_level(args.steps, 60.0)
+        r = {"zcps": c["value"], "cores": c["cores"], "steps": c["steps"], "ms_per_step": c["ms_per_step"],
+             "sample": c["sample"]}
+        label = TWO_LEVEL_LABEL
+    else:
+        r = time_oracle(args.workload, args.steps, args.warmup, budget_s=60.0)
+        label = WORKLOAD_LABELS.get(args.workload, args.workload)
     line = {"impl": "reference", "metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": r["zcps"],
             "unit": "zone-cycles/s", "n_gpus": args.gpus, "steps": r["steps"], "warmup": args.warmup,
             "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -534,6 +540,26 @@ def two_level_workload(small: bool = False):
     return pc, pf, origin
 
 
+def time_oracle_two_level(max_steps: int, budget_s: float):
+    """The oracle's two-level step on a bounded sample of the two-level workload (same wave, same operators)."""
+    from oracle import oracle as O
+    O.build()
+    qc, qf, qo = two_level_workload(small=True)
+    qf = replace(qf, nb=(1, 1, 1))
+    uc, uf = O.enforce(qc, I.linear_wave_data(qc))[0], O.enforce(qf, I.linear_wave_data(qf))[0]
+    t0 = time.perf_counter()
+    O.step_two_level(qc, qf, qf.n, qo, uc, uf, 1)
+    k = max(1, min(max_steps, int(budget_s / max(time.perf_counter() - t0, 1e-6))))
+    t0 = time.perf_counter()
+    O.step_two_level(qc, qf, qf.n, qo, uc, uf, k)
+    dt = time.perf_counter() - t0
+    qleaf = qc.ncells - qf.ncells // 8 + qf.ncells
+    return {"value": qleaf * k / dt, "unit": "zone-cycles/s", "cores": O.num_threads(), "kind": "oracle",
+            "steps": k, "ms_per_step": dt / k * 1e3,
+            "sample": f"coarse 32^3 in 8 blocks of 16^3 + one refined 16^3 block at coarse cell {qo}; {qleaf} leaf "
+                      f"zones x {k} two-level RK4 steps"}
+
+
 def run_two_level(args):
     import torch
     from paper_2409_10383_b200 import build, z4c
@@ -590,23 +616,7 @@ def run_two_level(args):
     # restriction: every fine active cell read once, every covered coarse cell written; prolongation: every fine ghost
     # cell outside the box written, ~0.4 coarse cells read per such cell (the layers of coarse nodes under the shell)
     exch_bytes = 8 * I.NF * (pf.ncells + covered) + 8 * I.NF * int(1.4 * fine_ghost_out)
-    cpu = None
-    if not args.no_cpu:
-        from oracle import oracle as O
-        O.build()
-        qc, qf, qo = two_level_workload(small=True)
-        qf = replace(qf, nb=(1, 1, 1))
-        uc, uf = O.enforce(qc, I.linear_wave_data(qc))[0], O.enforce(qf, I.linear_wave_data(qf))[0]
-        t0 = time.perf_counter()
-        O.step_two_level(qc, qf, qf.n, qo, uc, uf, 1)
-        k = max(1, min(1000, int(10.0 / max(time.perf_counter() - t0, 1e-6))))
-        t0 = time.perf_counter()
-        O.step_two_level(qc, qf, qf.n, qo, uc, uf, k)
-        dt = time.perf_counter() - t0
-        qleaf = qc.ncells - qf.ncells // 8 + qf.ncells
-        cpu = {"value": qleaf * k / dt, "unit": "zone-cycles/s", "cores": O.num_threads(), "kind": "oracle",
-               "sample": f"coarse 32^3 in 8 blocks of 16^3 + one refined 16^3 block at coarse cell {qo}; {qleaf} leaf "
-                         f"zones x {k} two-level RK4 steps"}
+    cpu = None if args.no_cpu else time_oracle_two_level(1000, 10.0)
     line = {"metric": "zone-cycles/s (fp64 Z4c RK4 step)", "value": leaf * K / (ms * 1e-3), "unit": "zone-cycles/s",
             "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
